@@ -1,0 +1,163 @@
+/* bathy.h -- C ABI of libbathy.so: B200 (sm_100a) interpolation of sonar depth soundings onto a
+ * regular grid by three methods -- bilinear, separable natural bicubic spline, ordinary kriging.
+ *
+ * The operations are those of "Towards Real-Time Interpolation for Enhanced AUV Deep Sea Mapping"
+ * (arxiv 2505.22675), cited below as PAPER.md:Lnn, with the readings listed in DESIGN.md.
+ *
+ * Conventions (every entry point):
+ *   - `d_*` arguments are DEVICE pointers owned by the caller; `h_*` arguments are HOST pointers.
+ *     The library never allocates or frees caller buffers and never keeps a caller pointer after
+ *     the call's work on `cuda_stream` has completed.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-
+ *     pointer calls are asynchronous on that stream and do not synchronise the host.  `*_host`
+ *     calls copy host->device, run the same kernels and copy device->host on that stream and
+ *     return after the stream has drained.
+ *   - Return value: 0 (BATHY_OK) or a negative bathy_status.  Argument errors are detected
+ *     synchronously and nothing is launched.  No exceptions, no global state besides the launch
+ *     counter, no environment variables; calls on distinct streams are thread-safe.
+ *   - A grid is row-major fp32 with leading dimension nx.  Node (i, j) -- i = row (y), j = column
+ *     (x) -- sits at x = x0 + j*dx, y = y0 + i*dy.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns BATHY_ERR_CUDA.
+ */
+#ifndef BATHY_H
+#define BATHY_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define BATHY_API __attribute__((visibility("default")))
+#else
+#define BATHY_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BATHY_OK                = 0,
+    BATHY_ERR_NULL          = -1,   /* a required pointer is NULL */
+    BATHY_ERR_GEOMETRY      = -2,   /* input grid nx<2 or ny<2, output nx<1 or ny<1, dx<=0 or dy<=0, non-finite */
+    BATHY_ERR_K             = -3,   /* k<1, k>BATHY_MAX_K or k>n */
+    BATHY_ERR_VARIOGRAM     = -4,   /* range<=0, sill<=0, nugget<0, nugget>sill, unknown model, non-finite */
+    BATHY_ERR_WORKSPACE     = -5,   /* workspace NULL or smaller than *_workspace_bytes() */
+    BATHY_ERR_CUDA          = -6,   /* a CUDA runtime call failed (no device, out of memory, launch error) */
+    BATHY_ERR_SIZE          = -7,   /* n<1 or n>2^31-1 soundings, or a grid with more than 2^31-1 nodes per row/column */
+    BATHY_ERR_INDEX         = -8    /* index handle NULL or not built by krige_build_index */
+} bathy_status;
+
+#define BATHY_MAX_K 64
+
+/* Regular grid geometry ("a given cell structure of existing points ... inside a
+ * larger grid"). */
+typedef struct {
+    int32_t nx, ny;
+    float   x0, y0, dx, dy;
+} grid_geom_t;
+
+/* Variogram.  model 0 = exponential exactly as printed at L157,
+ * gamma(h) = nugget + (sill-nugget)(1 - exp(-h/range)) (no factor 3); model 1 = spherical,
+ * gamma(h) = nugget + (sill-nugget)(1.5 h/range - 0.5 (h/range)^3) for 0<h<range, sill beyond.
+ * gamma(0) = 0 for both.  `sill` is the TOTAL sill (nugget included); nugget <= sill. */
+typedef struct {
+    int32_t model;
+    float   range, sill, nugget;
+} variogram_t;
+
+#define BATHY_VGM_EXPONENTIAL 0
+#define BATHY_VGM_SPHERICAL   1
+
+/* Opaque, library-owned, immutable after build; may be shared by concurrent krige_predict calls. */
+typedef struct krige_index krige_index_t;
+
+/* ---------------------------------------------------------------------------------------------
+ * interp_bilinear -- PAPER.md:L115-L134 (section III-A), formula at L132.
+ * For every node (I, J) of `out`: u = (x - in.x0)/in.dx, v = (y - in.y0)/in.dy (float64 from the
+ * fp32 fields); i = min(floor u, nx-2), t = u - i (same for j, s); result =
+ * (1-t)(1-s) Q11 + t(1-s) Q21 + (1-t)s Q12 + t s Q22 with Q11 = in[j][i], Q21 = in[j][i+1],
+ * Q12 = in[j+1][i], Q22 = in[j+1][i+1], evaluated in fp32.  Nodes outside the input extent
+ * (u<0, u>nx-1, v<0, v>ny-1) are NaN; a NaN corner makes the node NaN (the paper's bilinear "has no
+ * fallback", L182).
+ * d_in  [in.ny * in.nx] fp32, read only.   d_out [out.ny * out.nx] fp32, fully overwritten.
+ * d_in and d_out must not overlap. */
+BATHY_API int interp_bilinear(const float* d_in, grid_geom_t in, float* d_out, grid_geom_t out, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * interp_spline -- separable natural bicubic spline (BASELINE.json north_star; DESIGN.md reading
+ * D1: the paper's section III-B, uses the local Catmull-Rom cubic instead).
+ * 1-D operator on uniform knots with spacing h: second derivatives M with M_0 = M_{n-1} = 0 and
+ * M_{i-1} + 4 M_i + M_{i+1} = 6 (z_{i-1} - 2 z_i + z_{i+1}) / h^2 (batched tridiagonal solves);
+ * S = A z_i + B z_{i+1} + ((A^3-A) M_i + (B^3-B) M_{i+1}) h^2/6, A = 1-t, B = t.  2-D = the tensor
+ * product (rows in x, then columns in y).  Interval location, extent and NaN rules as bilinear.
+ * Precondition: d_in holds no NaN (a NaN poisons its whole row and column; not checked).
+ * d_workspace: device scratch of at least interp_spline_workspace_bytes(in, out) bytes, 256-byte
+ * aligned, contents undefined on return; may be reused by later calls on the same stream. */
+BATHY_API size_t interp_spline_workspace_bytes(grid_geom_t in, grid_geom_t out);
+BATHY_API int interp_spline(const float* d_in, grid_geom_t in, float* d_out, grid_geom_t out,
+                  void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * krige_build_index -- uniform-grid binning of the soundings for the neighbour search that
+ * replaces the paper's "nearest n valid candidate neighbors" helper: bounding box,
+ * cell id per sounding, histogram, exclusive scan, stable scatter of (x, y, z, original index).
+ * d_x, d_y, d_z [n] fp32 (SoA), n in [1, 2^31-1]; finite, no two soundings at identical (x, y)
+ * (kriging with duplicates is singular -- such nodes come out NaN, see krige_predict).
+ * cell_size: edge of a square cell in the units of x/y; 0 = automatic (about 8 soundings per cell).
+ * The soundings are copied into library-owned device memory: the caller may free d_x/d_y/d_z once
+ * the stream reaches this point.  The call synchronises `cuda_stream` once (to size the cell
+ * grid from the bounding box).  *out_index is released only by krige_free_index. */
+BATHY_API int krige_build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n,
+                      float cell_size, void* cuda_stream, krige_index_t** out_index);
+
+/* ---------------------------------------------------------------------------------------------
+ * krige_predict -- ordinary kriging (section III-C) at every node of `out`.
+ * Node coordinates are the fp32 values xq = fmaf(J, dx, x0), yq = fmaf(I, dy, y0).
+ *   neighbours : the k soundings with the smallest (key, original index), key =
+ *                fmaf(ddx, ddx, ddy*ddy) in fp32 with ddx = xq - x_i, ddy = yq - y_i;
+ *   covariances: C_ij = sill - gamma(h_ij), c0_i = sill - gamma(h_0i);
+ *   weights    : C lambda + mu 1 = c0, 1^T lambda = 1, the standard ordinary-kriging system
+ *                (what PAPER.md:L159-L165 solves "using Gaussian elimination"), here by Cholesky
+ *                of C and a Schur complement for mu;
+ *   estimate   : z_hat = sum_i lambda_i z_i.
+ * k in [1, min(BATHY_MAX_K, n)].
+ * d_zhat            [out.ny * out.nx] fp32, fully overwritten.
+ * d_nbr_or_null     [out.ny * out.nx * k] int32: original indices of the neighbours in ascending
+ *                   (key, index) order (parity/debug output), or NULL.
+ * d_failed_or_null  one int64 device counter, INCREMENTED by the number of nodes whose system was
+ *                   not positive definite (duplicate soundings); those nodes are written NaN.
+ *                   The caller zeroes it.  NULL = not counted.
+ * Tiles (BASELINE.json config 5) are calls with a sub-geometry: x0/y0 shifted to the tile's first
+ * node, nx/ny the tile size, d_zhat a tile buffer. */
+BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram_t vg, int32_t k,
+                  float* d_zhat, int32_t* d_nbr_or_null, int64_t* d_failed_or_null, void* cuda_stream);
+
+/* Releases an index (synchronises the device first).  NULL is a no-op. */
+BATHY_API void krige_free_index(krige_index_t* idx);
+
+/* Introspection of an index (host values, valid after build): number of soundings, cell size used,
+ * cell-grid dimensions. */
+BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell_size, int32_t* ncx, int32_t* ncy);
+
+/* ---------------------------------------------------------------------------------------------
+ * Host-buffer forms: the same operations for callers whose data lives in host memory.  Each
+ * allocates device scratch, copies h_in (or h_x/h_y/h_z) to the device, runs the kernels of the
+ * device-pointer form, copies the result back and waits for the stream.  Pinned host memory makes
+ * the copies asynchronous and faster but is not required. */
+BATHY_API int interp_bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
+BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
+BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
+               grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
+               void* cuda_stream);
+
+/* Static, never NULL. */
+BATHY_API const char* bathy_strerror(int status);
+
+/* Number of kernel launches the library has issued in this process (monotonic; for bench.py's
+ * gpu_launches and tests). */
+BATHY_API int64_t bathy_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BATHY_H */

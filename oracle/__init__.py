@@ -158,9 +158,12 @@ class Buckets:
             raise ValueError("oracle_buckets_build failed")
 
     def __del__(self):
-        if getattr(self, "h", None):
-            lib().oracle_buckets_free(self.h)
-            self.h = None
+        try:
+            if getattr(self, "h", None):
+                lib().oracle_buckets_free(self.h)
+                self.h = None
+        except Exception:          # interpreter shutdown
+            pass
 
 
 def knn(x, y, xq, yq, k, buckets: Buckets | None = None):

@@ -1,0 +1,9 @@
+"""bathy-b200: B200-native (sm_100a) bilinear / natural-bicubic-spline / ordinary-kriging
+interpolation of sonar soundings onto a grid -- the data-parallel hot path of arxiv 2505.22675.
+
+Public API = the C ABI of include/bathy.h, re-exported by `binding` under the same names.
+"""
+from .binding import (EXPONENTIAL, SPHERICAL, MAX_K, BathyError, KrigeIndex, interp_bilinear,  # noqa: F401
+                      interp_bilinear_host, interp_spline, interp_spline_host, interp_spline_workspace_bytes,
+                      krige_build_index, krige_free_index, krige_host, krige_predict, launch_count, lib)
+from .workloads import Geom  # noqa: F401

@@ -1,0 +1,236 @@
+"""Thin Python binding of libbathy.so (include/bathy.h): argument marshalling only.
+
+Same names as the C ABI.  torch is used for device memory and streams; every step of the path
+runs in the library's CUDA kernels.  There is no CPU fallback: if the shared library is missing
+or cannot be loaded, importing a symbol raises, and compute calls without a CUDA device fail
+with BATHY_ERR_CUDA.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from .workloads import Geom
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbathy.so")
+
+EXPONENTIAL, SPHERICAL = 0, 1
+MAX_K = 64
+
+SYMBOLS = ["interp_bilinear", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
+           "krige_predict", "krige_free_index", "krige_index_info", "interp_bilinear_host",
+           "interp_spline_host", "krige_host", "bathy_strerror", "bathy_launch_count"]
+
+
+class GridGeom(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("x0", C.c_float), ("y0", C.c_float),
+                ("dx", C.c_float), ("dy", C.c_float)]
+
+
+class Variogram(C.Structure):
+    _fields_ = [("model", C.c_int32), ("range", C.c_float), ("sill", C.c_float), ("nugget", C.c_float)]
+
+
+class BathyError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {lib().bathy_strerror(status).decode()} ({status})")
+
+
+_lib = None
+
+
+def lib():
+    """Loads libbathy.so (build it with `python -m paper_2505_22675_b200.build`); fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build the CUDA extension first "
+                              "(python -m paper_2505_22675_b200.build); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp = C.c_void_p
+        L.interp_bilinear.argtypes = [vp, GridGeom, vp, GridGeom, vp]
+        L.interp_spline_workspace_bytes.argtypes = [GridGeom, GridGeom]
+        L.interp_spline_workspace_bytes.restype = C.c_size_t
+        L.interp_spline.argtypes = [vp, GridGeom, vp, GridGeom, vp, C.c_size_t, vp]
+        L.krige_build_index.argtypes = [vp, vp, vp, C.c_int64, C.c_float, vp, C.POINTER(vp)]
+        L.krige_predict.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, vp, vp, vp]
+        L.krige_free_index.argtypes = [vp]
+        L.krige_free_index.restype = None
+        L.krige_index_info.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_float),
+                                       C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.interp_bilinear_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
+        L.interp_spline_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
+        L.krige_host.argtypes = [vp, vp, vp, C.c_int64, C.c_float, GridGeom, Variogram, C.c_int32, vp, vp, vp]
+        L.bathy_strerror.argtypes = [C.c_int]
+        L.bathy_strerror.restype = C.c_char_p
+        L.bathy_launch_count.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def _geom(g) -> GridGeom:
+    if isinstance(g, GridGeom):
+        return g
+    return GridGeom(int(g.nx), int(g.ny), float(g.x0), float(g.y0), float(g.dx), float(g.dy))
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _check(rc: int, where: str):
+    if rc != 0:
+        raise BathyError(rc, where)
+
+
+def _dev_f32(t: torch.Tensor, name: str) -> torch.Tensor:
+    if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float32 CUDA tensor")
+    return t
+
+
+def launch_count() -> int:
+    return int(lib().bathy_launch_count())
+
+
+def interp_bilinear(z: torch.Tensor, gin, gout, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """PAPER.md:L115-L134.  z [ny_in, nx_in] fp32 on the GPU -> [ny_out, nx_out]."""
+    gi, go = _geom(gin), _geom(gout)
+    _dev_f32(z, "z")
+    assert z.numel() == gi.nx * gi.ny
+    if out is None:
+        out = torch.empty((go.ny, go.nx), dtype=torch.float32, device=z.device)
+    _dev_f32(out, "out")
+    assert out.numel() == go.nx * go.ny
+    _check(lib().interp_bilinear(z.data_ptr(), gi, out.data_ptr(), go, _stream(stream)), "interp_bilinear")
+    return out
+
+
+def interp_spline_workspace_bytes(gin, gout) -> int:
+    return int(lib().interp_spline_workspace_bytes(_geom(gin), _geom(gout)))
+
+
+def interp_spline(z: torch.Tensor, gin, gout, out: torch.Tensor | None = None,
+                  workspace: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """Separable natural bicubic spline (reading D1)."""
+    gi, go = _geom(gin), _geom(gout)
+    _dev_f32(z, "z")
+    assert z.numel() == gi.nx * gi.ny
+    if out is None:
+        out = torch.empty((go.ny, go.nx), dtype=torch.float32, device=z.device)
+    _dev_f32(out, "out")
+    need = interp_spline_workspace_bytes(gi, go)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=z.device)
+    _check(lib().interp_spline(z.data_ptr(), gi, out.data_ptr(), go, workspace.data_ptr(),
+                               workspace.numel() * workspace.element_size(), _stream(stream)), "interp_spline")
+    return out
+
+
+class KrigeIndex:
+    """Owner of an opaque krige_index_t*."""
+
+    def __init__(self, handle: int):
+        self.handle = handle
+
+    def info(self) -> dict:
+        n, c, ncx, ncy = C.c_int64(), C.c_float(), C.c_int32(), C.c_int32()
+        _check(lib().krige_index_info(self.handle, C.byref(n), C.byref(c), C.byref(ncx), C.byref(ncy)), "krige_index_info")
+        return {"n": n.value, "cell_size": c.value, "ncx": ncx.value, "ncy": ncy.value}
+
+    def free(self):
+        if self.handle:
+            lib().krige_free_index(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def krige_build_index(x: torch.Tensor, y: torch.Tensor, z: torch.Tensor, cell_size: float = 0.0,
+                      stream=None) -> KrigeIndex:
+    for t, nm in ((x, "x"), (y, "y"), (z, "z")):
+        _dev_f32(t, nm)
+    assert x.numel() == y.numel() == z.numel()
+    h = C.c_void_p()
+    _check(lib().krige_build_index(x.data_ptr(), y.data_ptr(), z.data_ptr(), x.numel(), float(cell_size),
+                                   _stream(stream), C.byref(h)), "krige_build_index")
+    return KrigeIndex(h.value)
+
+
+def krige_predict(index: KrigeIndex, gout, model: int, range_: float, sill: float, nugget: float, k: int,
+                  out: torch.Tensor | None = None, want_nbr: bool = False, failed: torch.Tensor | None = None,
+                  stream=None):
+    """PAPER.md:L146-L171.  Returns zhat [ny, nx] (and nbr [ny, nx, k] int32 when want_nbr)."""
+    go = _geom(gout)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if out is None:
+        out = torch.empty((go.ny, go.nx), dtype=torch.float32, device=dev)
+    _dev_f32(out, "out")
+    nbr = torch.empty((go.ny, go.nx, int(k)), dtype=torch.int32, device=dev) if want_nbr else None
+    vg = Variogram(int(model), float(range_), float(sill), float(nugget))
+    _check(lib().krige_predict(index.handle, go, vg, int(k), out.data_ptr(),
+                               nbr.data_ptr() if nbr is not None else None,
+                               failed.data_ptr() if failed is not None else None, _stream(stream)), "krige_predict")
+    return (out, nbr) if want_nbr else out
+
+
+def krige_free_index(index: KrigeIndex) -> None:
+    index.free()
+
+
+# ---- host-buffer forms (numpy in, numpy out; copies happen inside the C call)
+
+def _host_f32(a, name):
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous():
+            raise TypeError(f"{name} must be a contiguous float32 host tensor")
+        return a, a.data_ptr()
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data
+
+
+def interp_bilinear_host(z, gin, gout, out=None, stream=None):
+    gi, go = _geom(gin), _geom(gout)
+    z, zp = _host_f32(z, "z")
+    if out is None:
+        out = np.empty((go.ny, go.nx), dtype=np.float32)
+    out, op = _host_f32(out, "out")
+    _check(lib().interp_bilinear_host(zp, gi, op, go, _stream(stream)), "interp_bilinear_host")
+    return out
+
+
+def interp_spline_host(z, gin, gout, out=None, stream=None):
+    gi, go = _geom(gin), _geom(gout)
+    z, zp = _host_f32(z, "z")
+    if out is None:
+        out = np.empty((go.ny, go.nx), dtype=np.float32)
+    out, op = _host_f32(out, "out")
+    _check(lib().interp_spline_host(zp, gi, op, go, _stream(stream)), "interp_spline_host")
+    return out
+
+
+def krige_host(x, y, z, gout, model, range_, sill, nugget, k, cell_size: float = 0.0, out=None, stream=None):
+    go = _geom(gout)
+    x, xp = _host_f32(x, "x")
+    y, yp = _host_f32(y, "y")
+    z, zp = _host_f32(z, "z")
+    if out is None:
+        out = np.empty((go.ny, go.nx), dtype=np.float32)
+    out, op = _host_f32(out, "out")
+    failed = C.c_int64(0)
+    vg = Variogram(int(model), float(range_), float(sill), float(nugget))
+    n = x.numel() if isinstance(x, torch.Tensor) else x.shape[0]
+    _check(lib().krige_host(xp, yp, zp, n, float(cell_size), go, vg, int(k), op, C.addressof(failed),
+                            _stream(stream)), "krige_host")
+    return out, failed.value

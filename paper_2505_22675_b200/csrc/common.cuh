@@ -1,0 +1,92 @@
+// common.cuh -- shared plumbing of libbathy.so (CUDA path only; the oracle shares nothing with this).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <math.h>
+#include "../../include/bathy.h"
+
+namespace bathy {
+
+constexpr int kSMs = 148;            // B200: 2 dies x 74 SMs
+
+void count_launch(int n = 1);        // api.cu: backs bathy_launch_count()
+
+#define BATHY_CUDA_TRY(expr)                         \
+    do {                                             \
+        cudaError_t e__ = (expr);                    \
+        if (e__ != cudaSuccess) return BATHY_ERR_CUDA; \
+    } while (0)
+
+inline int launch_status() { return cudaGetLastError() == cudaSuccess ? BATHY_OK : BATHY_ERR_CUDA; }
+
+inline bool finite_f(float v) { return isfinite(v); }
+
+inline int check_in_geom(const grid_geom_t& g)
+{
+    if (g.nx < 2 || g.ny < 2) return BATHY_ERR_GEOMETRY;
+    if (!finite_f(g.x0) || !finite_f(g.y0) || !finite_f(g.dx) || !finite_f(g.dy)) return BATHY_ERR_GEOMETRY;
+    if (!(g.dx > 0.0f) || !(g.dy > 0.0f)) return BATHY_ERR_GEOMETRY;
+    return BATHY_OK;
+}
+
+inline int check_out_geom(const grid_geom_t& g)
+{
+    if (g.nx < 1 || g.ny < 1) return BATHY_ERR_GEOMETRY;
+    if (!finite_f(g.x0) || !finite_f(g.y0) || !finite_f(g.dx) || !finite_f(g.dy)) return BATHY_ERR_GEOMETRY;
+    if (!(g.dx > 0.0f) || !(g.dy > 0.0f)) return BATHY_ERR_GEOMETRY;
+    return BATHY_OK;
+}
+
+// One axis of the output->input index map (readings B1/B2): u = ((o0 + J*od) - i0) / id in float64
+// from the fp32 geometry fields, each operation rounded separately (no contraction) so that the
+// interval decision is taken in the same precision as the definition.
+struct AxisMap {
+    double o0, od, i0, id;
+    int n_in, n_out;
+};
+
+inline AxisMap axis_x(const grid_geom_t& in, const grid_geom_t& out)
+{
+    return AxisMap{(double)out.x0, (double)out.dx, (double)in.x0, (double)in.dx, in.nx, out.nx};
+}
+inline AxisMap axis_y(const grid_geom_t& in, const grid_geom_t& out)
+{
+    return AxisMap{(double)out.y0, (double)out.dy, (double)in.y0, (double)in.dy, in.ny, out.ny};
+}
+
+__device__ __forceinline__ double axis_u(const AxisMap& m, int J)
+{
+    double x = __dadd_rn(m.o0, __dmul_rn((double)J, m.od));
+    return __ddiv_rn(__dsub_rn(x, m.i0), m.id);
+}
+
+// Interval index (or -1 when the node is outside the input extent) and local coordinate t.
+__device__ __forceinline__ int axis_locate(const AxisMap& m, int J, float* t)
+{
+    double u = axis_u(m, J);
+    if (!(u >= 0.0) || !(u <= (double)(m.n_in - 1))) { *t = 0.0f; return -1; }
+    int i = (int)floor(u);
+    i = min(i, m.n_in - 2);
+    i = max(i, 0);
+    *t = (float)(u - (double)i);
+    return i;
+}
+
+// Interval index clamped into [0, n_in-2] whatever u is (footprint bounds of a tile).
+__device__ __forceinline__ int axis_clamped(const AxisMap& m, int J)
+{
+    double u = axis_u(m, J);
+    if (!(u >= 0.0)) return 0;
+    if (u >= (double)(m.n_in - 1)) return m.n_in - 2;
+    return min((int)floor(u), m.n_in - 2);
+}
+
+// Host-side bound on the input footprint (in samples) of `n_nodes` consecutive output nodes.
+inline long long footprint_bound(const AxisMap& m, int n_nodes)
+{
+    double span = (double)(n_nodes - 1) * m.od / m.id;
+    if (!(span < 1e9)) return (long long)2e9;
+    return (long long)floor(span) + 3;        // floor(u_last) - floor(u_first) <= floor(span)+1, +1 sample, +1 slack
+}
+
+}  // namespace bathy

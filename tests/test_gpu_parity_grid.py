@@ -1,0 +1,144 @@
+"""GPU parity, through the C ABI, of interp_bilinear and interp_spline against the float64 oracle.
+Tolerance (BASELINE.json north_star): max abs error <= 1e-5 x depth range of the oracle output."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2505_22675_b200 import workloads as W
+from _util import ogeom, depth_range, max_abs_err
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+def _bathy():
+    import paper_2505_22675_b200 as b
+    return b
+
+
+def _run(method, z, gi, go):
+    b = _bathy()
+    zt = torch.from_numpy(np.ascontiguousarray(z)).cuda()
+    fn = b.interp_bilinear if method == "bilinear" else b.interp_spline
+    out = fn(zt, gi, go)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _ref(method, z, gi, go):
+    return (oracle.bilinear if method == "bilinear" else oracle.spline)(z, ogeom(gi), ogeom(go))
+
+
+def _filled_config1():
+    """Config 1 grid with its NaN cells filled by the ORACLE's kriging (isolates the method)."""
+    w = W.grid_config(1)
+    x, y, z = W.grid_to_scattered(w.z)
+    v = oracle.vgm(oracle.SPHERICAL, 10.0, W.sample_variance(z), 0.0)
+    ii, jj = np.nonzero(w.nan_mask)
+    r = oracle.krige_points(x, y, z, jj.astype(np.float32), ii.astype(np.float32), v, 8)
+    filled = w.z.copy()
+    filled[ii, jj] = r["zhat"].astype(np.float32)
+    assert not np.isnan(filled).any()
+    return w, filled
+
+
+@pytest.mark.parametrize("method", ["bilinear", "spline"])
+def test_config1(method):
+    w, filled = _filled_config1()
+    ref = _ref(method, filled, w.geom_in, w.geom_out)
+    got = _run(method, filled, w.geom_in, w.geom_out)
+    err = max_abs_err(got, ref)
+    assert err <= TOL * depth_range(ref), (err, depth_range(ref))
+    if method == "bilinear":
+        assert np.array_equal(got[::4, ::4], filled)            # knots bit-exact
+
+
+@pytest.mark.parametrize("method", ["bilinear", "spline"])
+@pytest.mark.parametrize("config,n_in,factor,nf", [(2, 257, 4, 40), (3, 600, 2, 200)])
+def test_reduced_configs_2_3(method, config, n_in, factor, nf):
+    # same generator, reduced size: several tiles in both directions and a ragged tail
+    w = W.grid_config(config, n_in=n_in, factor=factor, n_features=nf)
+    ref = _ref(method, w.z, w.geom_in, w.geom_out)
+    got = _run(method, w.z, w.geom_in, w.geom_out)
+    err = max_abs_err(got, ref)
+    assert err <= TOL * depth_range(ref), (err, depth_range(ref))
+
+
+@pytest.mark.parametrize("method", ["bilinear", "spline"])
+def test_general_geometry_and_out_of_extent(method):
+    rng = np.random.default_rng(21)
+    z = (rng.normal(-3000, 40, (37, 53))).astype(np.float32)
+    gi = W.Geom(53, 37, 10.0, -5.0, 2.0, 3.0)
+    # non-integer ratio, shifted origin, nodes outside on all four sides
+    go = W.Geom(301, 173, 4.0, -9.5, 0.37, 0.71)
+    ref = _ref(method, z, gi, go)
+    got = _run(method, z, gi, go)
+    assert np.isnan(ref).any() and np.isfinite(ref).any()
+    err = max_abs_err(got, ref)
+    assert err <= TOL * depth_range(ref), (err, depth_range(ref))
+    # down-sampling (footprint larger than a tile: gather path)
+    z2 = rng.normal(-3000, 40, (400, 900)).astype(np.float32)
+    gi2 = W.Geom(900, 400, 0.0, 0.0, 1.0, 1.0)
+    go2 = W.Geom(40, 30, 0.5, 0.25, 22.0, 13.0)
+    ref2 = _ref(method, z2, gi2, go2)
+    got2 = _run(method, z2, gi2, go2)
+    assert max_abs_err(got2, ref2) <= TOL * depth_range(ref2)
+
+
+@pytest.mark.parametrize("method", ["bilinear", "spline"])
+def test_degenerate_sizes(method):
+    rng = np.random.default_rng(22)
+    for (ny, nx), (oy, ox) in [((2, 2), (5, 7)), ((2, 9), (1, 33)), ((9, 2), (17, 1)), ((3, 3), (1, 1))]:
+        z = rng.normal(-100, 5, (ny, nx)).astype(np.float32)
+        gi = W.Geom(nx, ny, 0.0, 0.0, 1.0, 1.0)
+        go = W.Geom(ox, oy, 0.0, 0.0, (nx - 1) / max(ox - 1, 1), (ny - 1) / max(oy - 1, 1))
+        ref = _ref(method, z, gi, go)
+        got = _run(method, z, gi, go)
+        assert max_abs_err(got, ref) <= TOL * max(depth_range(ref), 1.0)
+
+
+def test_bilinear_nan_propagation():
+    w = W.grid_config(1)                                          # 10 % NaN cells, not filled
+    ref = oracle.bilinear(w.z, ogeom(w.geom_in), ogeom(w.geom_out))
+    got = _run("bilinear", w.z, w.geom_in, w.geom_out)
+    assert np.isnan(ref).sum() > 0
+    err = max_abs_err(got, ref)                                   # also checks the NaN pattern (B4)
+    assert err <= TOL * depth_range(ref)
+
+
+def test_plane_and_constant_exactness():
+    # linear fields are reproduced by both methods (all second derivatives vanish)
+    X, Y = np.meshgrid(np.arange(70, dtype=np.float64), np.arange(50, dtype=np.float64))
+    z = (-5000 + 0.5 * X + 0.25 * Y).astype(np.float32)
+    gi, go = W.Geom(70, 50, 0, 0, 1, 1), W.Geom(277, 197, 0, 0, 0.25, 0.25)
+    Xo, Yo = np.meshgrid(np.arange(277) * 0.25, np.arange(197) * 0.25)
+    exact = -5000 + 0.5 * Xo + 0.25 * Yo
+    for method in ("bilinear", "spline"):
+        got = _run(method, z, gi, go)
+        assert np.abs(got - exact).max() <= 1e-3, method             # ~2 ulp at 5000 m
+
+
+def test_argument_errors_and_workspace():
+    b = _bathy()
+    z = torch.zeros((4, 4), device="cuda")
+    with pytest.raises(b.BathyError) as e:
+        b.interp_bilinear(z, W.Geom(4, 4, 0, 0, 0.0, 1), W.Geom(4, 4, 0, 0, 1, 1))
+    assert e.value.status == -2
+    with pytest.raises(b.BathyError):
+        b.interp_bilinear(torch.zeros((1, 16), device="cuda"), W.Geom(16, 1, 0, 0, 1, 1), W.Geom(4, 4, 0, 0, 1, 1))
+    need = b.interp_spline_workspace_bytes(W.Geom(4, 4, 0, 0, 1, 1), W.Geom(7, 7, 0, 0, .5, .5))
+    assert need > 0
+    with pytest.raises(b.BathyError) as e:
+        b.interp_spline(z, W.Geom(4, 4, 0, 0, 1, 1), W.Geom(7, 7, 0, 0, .5, .5),
+                        workspace=torch.empty(max(need - 256, 1), dtype=torch.uint8, device="cuda"))
+    assert e.value.status == -5
+
+
+def test_host_forms_match_device_forms():
+    b = _bathy()
+    w = W.grid_config(2, n_in=129, factor=4, n_features=10)
+    for method, hostfn in (("bilinear", b.interp_bilinear_host), ("spline", b.interp_spline_host)):
+        dev = _run(method, w.z, w.geom_in, w.geom_out)
+        host = hostfn(w.z, w.geom_in, w.geom_out)
+        assert np.array_equal(dev, host)
