@@ -1,0 +1,420 @@
+#!/usr/bin/env python
+"""bench.py -- output nodes/s of the hot path (bilinear, natural bicubic spline, ordinary kriging)
+on B200, with the roofline of the dominant kernel and the oracle timed beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A STEP is one pass of the whole hot path (every row of SURVEY.md 8(a)) over one batch of seeded
+synthetic input:
+    interp_bilinear   config 3   4096^2 -> 8191^2 fp32                       (B1)
+    interp_spline     config 3   4096^2 -> 8191^2 fp32                       (S1-S4)
+    krige_build_index config 4   ~1.0 M multibeam soundings                   (K1)
+    krige_predict     config 4   -> 2048^2 nodes, k=32, exponential a=50 m    (K2-K5)
+`value` = output nodes of all three methods per second of device time, inputs resident in HBM.
+`methods` gives nodes/s and the roofline of each method separately (BASELINE.json's metric is
+per method); `roofline` is the one of the kernel that takes most of the step.
+`e2e` is the same step through the C ABI's host-buffer entry points (pinned host memory, the
+host<->device copies inside the timed region).
+Other workloads (`--workload small|config2|config5`) run the same code on the other configs.
+
+N > 1 (torchrun): every rank runs the same step on its own batch (seed + rank): the path shards
+by batch with no data-path collective ("weak").  Time = max over ranks.
+
+`--impl reference` times the float64 CPU oracle (oracle/, as it stands) on a bounded sample of the
+same workload -- this tier has no reference implementation to install.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "output nodes/s (bilinear + natural bicubic spline + ordinary kriging, one pass of the hot path)"
+UNIT = "nodes/s"
+FP32_LANES_PER_SM, SMS = 128, 148          # guide: 4 SMSP x 32 FP32 lanes, 148 SMs
+
+
+def krige_flops(k: int) -> float:
+    """Algorithmic flop per kriging node: Cholesky k^3/3,
+    two right-hand sides forward+back 4k^2, covariances 10 flop-equivalents for each of the
+    k(k+1)/2 pairs, 10k for c0 and the estimate."""
+    return k ** 3 / 3.0 + 4.0 * k * k + 5.0 * k * (k + 1) + 10.0 * k
+
+
+WORKLOADS = {
+    # name: (grid config, n_in, factor, features | kriging config, width, n_target, n_out)
+    "default": dict(grid=(3, 4096, 2, 8000), krige=(4, 2000.0, 1_000_000, 2048), tiles=False,
+                    label="config3(bilinear+spline 4096^2->8191^2) + config4(kriging 1.0M soundings->2048^2, k=32 exponential)"),
+    "config2": dict(grid=(2, 1024, 4, 500), krige=(4, 2000.0, 1_000_000, 2048), tiles=False,
+                    label="config2(bilinear+spline 1024^2->4093^2) + config4(kriging)"),
+    "config5": dict(grid=(3, 4096, 2, 8000), krige=(5, 4000.0, 4_000_000, 4096), tiles=True,
+                    label="config3(bilinear+spline) + config5(kriging 4.0M soundings->4096^2 as 64 tiles of 512^2, k=64 spherical)"),
+    "small": dict(grid=(2, 257, 4, 40), krige=(4, 250.0, 15625, 200), tiles=False,
+                  label="reduced configs (257^2->1025^2; 15.6k soundings->200^2, k=32)"),
+}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for (_, r) in self.rows]
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            f = [c.strip() for c in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ inputs
+
+def make_inputs(name: str, rank: int):
+    from paper_2505_22675_b200 import workloads as W
+    spec = WORKLOADS[name]
+    gc, n_in, factor, nf = spec["grid"]
+    kc, width, n_target, n_out = spec["krige"]
+    gw = W.grid_config(gc, n_in=n_in, factor=factor, n_features=nf, seed=W.SEEDS[gc] + 100 * rank)
+    sw = W.sounding_config(kc, width=width, n_target=n_target, n_out=n_out, seed=W.SEEDS[kc] + 100 * rank)
+    if spec["tiles"]:
+        tiles = W.boustrophedon_tiles(n_out, max(n_out // 8, 1))
+    else:
+        tiles = [(0, 0, n_out, n_out)]
+    return gw, sw, tiles
+
+
+# ------------------------------------------------------------------------------------------ our arm
+
+def run_ours(args):
+    import torch
+    import paper_2505_22675_b200 as B
+    from paper_2505_22675_b200 import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()                                             # fails loudly if libbathy.so is missing
+
+    gw, sw, tiles = make_inputs(args.workload, rank)
+    gi, go, gk = gw.geom_in, gw.geom_out, sw.geom_out
+    n_grid, n_krige = go.n, gk.n
+    nodes_per_step = 2 * n_grid + n_krige
+
+    # resident inputs and outputs
+    z_in = torch.from_numpy(gw.z).to(dev)
+    out_b = torch.empty(go.shape, dtype=torch.float32, device=dev)
+    out_s = torch.empty(go.shape, dtype=torch.float32, device=dev)
+    ws = torch.empty(B.interp_spline_workspace_bytes(gi, go), dtype=torch.uint8, device=dev)
+    sx, sy, sz = (torch.from_numpy(a).to(dev) for a in (sw.x, sw.y, sw.z))
+    out_k = torch.empty(gk.shape, dtype=torch.float32, device=dev)
+    failed = torch.zeros(1, dtype=torch.int64, device=dev)
+    tile_geoms = [(W.tile_geom(gk, i0, j0, ny, nx), i0, j0, ny, nx) for (i0, j0, ny, nx) in tiles]
+    tile_bufs = [torch.empty((ny, nx), dtype=torch.float32, device=dev) for (_, _, _, ny, nx) in tile_geoms] \
+        if len(tiles) > 1 else None
+    stream = torch.cuda.current_stream()
+
+    def step(ev=None):
+        if ev: ev[0].record(stream)
+        B.interp_bilinear(z_in, gi, go, out=out_b)
+        if ev: ev[1].record(stream)
+        B.interp_spline(z_in, gi, go, out=out_s, workspace=ws)
+        if ev: ev[2].record(stream)
+        idx = B.krige_build_index(sx, sy, sz)
+        if ev: ev[3].record(stream)
+        if tile_bufs is None:
+            B.krige_predict(idx, gk, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=out_k, failed=failed)
+        else:                                           # config 5: 64 calls in arrival order
+            for (tg, i0, j0, ny, nx), buf in zip(tile_geoms, tile_bufs):
+                B.krige_predict(idx, tg, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=buf, failed=failed)
+        if ev: ev[4].record(stream)
+        return idx
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step().free()
+    barrier()
+
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    sampler = ClockSampler(local) if rank == 0 else None
+    n0 = B.launch_count()
+    t0 = time.time()
+    barrier()
+    idxs = []
+    for s in range(args.steps):
+        idxs.append(step(evs[s]))
+    barrier()
+    t1 = time.time()
+    n1 = B.launch_count()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    for i in idxs:
+        i.free()
+    assert int(failed.item()) == 0, "kriging reported failed nodes on the bench workload"
+
+    seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])        # ms per segment
+    total_ms = float(evs[0][0].elapsed_time(evs[-1][4]))
+    t = torch.tensor([total_ms] + seg.mean(axis=0).tolist(), dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, ms_bil, ms_spl, ms_idx, ms_krg = t.tolist()
+    ms_per_step = total_ms / args.steps
+
+    # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the timed region)
+    hz = torch.from_numpy(gw.z).pin_memory()
+    hob = torch.empty(go.shape, dtype=torch.float32).pin_memory()
+    hos = torch.empty(go.shape, dtype=torch.float32).pin_memory()
+    hx, hy, hzz = (torch.from_numpy(a).pin_memory() for a in (sw.x, sw.y, sw.z))
+    hok = torch.empty(gk.shape, dtype=torch.float32).pin_memory()
+
+    def e2e_step():
+        B.interp_bilinear_host(hz, gi, go, out=hob)
+        B.interp_spline_host(hz, gi, go, out=hos)
+        _, nfail = B.krige_host(hx, hy, hzz, gk, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=hok)
+        return float(hok[0, 0]) + float(hob[0, 0]) + float(hos[0, 0]) + nfail      # the host reads the result
+
+    e2e_steps = max(2, min(args.steps, 5))
+    e2e_step()
+    barrier()
+    te0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    barrier()
+    e2e_ms = (time.perf_counter() - te0) * 1e3 / e2e_steps
+    te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_ms = float(te.item())
+    h2d = 2 * gi.n * 4 + 3 * sw.x.shape[0] * 4
+    d2h = 2 * n_grid * 4 + n_krige * 4 + 8
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks = load_peaks()
+    fp32_peak = SMS * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12     # TFLOP/s at the max SM clock
+    grid_bytes = 4.0 * (gi.n + n_grid)                  # compulsory: input read once, output written once
+    kf = krige_flops(sw.k)
+    meth = {
+        "bilinear": {"nodes_per_s": n_grid / (ms_bil * 1e-3), "ms": ms_bil, "launches": 1,
+                     "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_bil * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                  "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid}},
+        "spline": {"nodes_per_s": n_grid / (ms_spl * 1e-3), "ms": ms_spl,
+                   "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_spl * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid,
+                                "note": "whole call (all its kernels) against the compulsory bytes of the method"}},
+        "krige_build_index": {"soundings_per_s": sw.x.shape[0] / (ms_idx * 1e-3), "ms": ms_idx},
+        "kriging": {"nodes_per_s": n_krige / (ms_krg * 1e-3), "ms": ms_krg, "k": sw.k, "launches": len(tiles),
+                    "roofline": {"bound": "alu", "achieved": kf * n_krige / (ms_krg * 1e-3) / 1e12, "peak": fp32_peak,
+                                 "unit": "TFLOP/s", "flop_per_node": kf}},
+    }
+    for m in ("bilinear", "spline", "kriging"):
+        r = meth[m]["roofline"]
+        r["frac"] = r["achieved"] / r["peak"]
+    dom = max(("bilinear", "spline", "kriging"), key=lambda m: meth[m]["ms"])
+    kernel_name = {"bilinear": "bilinear_tiled_kernel", "spline": "interp_spline (all kernels)",
+                   "kriging": "krige_predict_kernel"}[dom]
+    roof = dict(meth[dom]["roofline"])
+    roof.update({"kernel": kernel_name, "traffic": None, "peak_source": (
+        f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else
+        f"derived: {SMS} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)")})
+    tr = os.path.join(ROOT, "profiles", "traffic.json")      # DRAM bytes per launch from the committed ncu capture
+    if os.path.exists(tr):
+        try:
+            with open(tr) as f:
+                roof["traffic"] = json.load(f).get(args.workload, {}).get(dom)
+        except Exception:
+            pass
+
+    line = {
+        "metric": METRIC, "value": world * nodes_per_step / (ms_per_step * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.workload]["label"], "nodes_per_step_per_gpu": nodes_per_step,
+                   "soundings": int(sw.x.shape[0]), "k": sw.k,
+                   "l2": "grid inputs+outputs (%.0f MB per method) exceed the 126 MB L2; no flush" % (grid_bytes / 1e6)
+                   if grid_bytes > 2.0e8 else "grid data fits L2: warm-L2 numbers for bilinear/spline",
+                   "parallelism": f"replicated batches x{world}, no collective"},
+        "methods": meth,
+        "roofline": roof,
+        "e2e": {"value": world * nodes_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                "api": "interp_bilinear_host + interp_spline_host + krige_host (pinned host buffers)"},
+        "gpu_launches": int(n1 - n0),
+        "clocks": clocks,
+    }
+    if args.cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(args.workload, budget_s=args.cpu_budget)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------------------------------ oracle arm
+
+def oracle_sample_step(name: str, gw, sw, krige_nodes: int, grid_n_in: int):
+    """One bounded sample of the step through the float64 oracle: bilinear and spline on the
+    top-left grid_n_in^2 crop of the input (same up-sampling factor), kriging at krige_nodes nodes
+    spread evenly over the output grid (full sounding set).  Returns seconds per method and the
+    nodes each processed."""
+    import oracle
+    from paper_2505_22675_b200 import workloads as W
+    gi, go = gw.geom_in, gw.geom_out
+    n = min(grid_n_in, gi.nx)
+    factor = round(gi.dx / go.dx)
+    crop = np.ascontiguousarray(gw.z[:n, :n])
+    ogi = oracle.geom(n, n, gi.x0, gi.y0, gi.dx, gi.dy)
+    n_out = (n - 1) * factor + 1
+    ogo = oracle.geom(n_out, n_out, go.x0, go.y0, go.dx, go.dy)
+    t0 = time.perf_counter(); oracle.bilinear(crop, ogi, ogo); t_b = time.perf_counter() - t0
+    t0 = time.perf_counter(); oracle.spline(crop, ogi, ogo); t_s = time.perf_counter() - t0
+    gk = sw.geom_out
+    v = oracle.vgm(sw.model, sw.range_, sw.sill, sw.nugget)
+    t0 = time.perf_counter()
+    buckets = oracle.Buckets(sw.x, sw.y, 4.0)
+    xq, yq = oracle.node_coords(oracle.geom(gk.nx, gk.ny, gk.x0, gk.y0, gk.dx, gk.dy))
+    sel = np.linspace(0, gk.n - 1, min(krige_nodes, gk.n)).astype(np.int64)
+    oracle.krige_points(sw.x, sw.y, sw.z, xq.ravel()[sel], yq.ravel()[sel], v, sw.k, buckets, want_nbr=False)
+    t_k = time.perf_counter() - t0
+    return {"bilinear": (t_b, n_out * n_out), "spline": (t_s, n_out * n_out), "kriging": (t_k, sel.shape[0])}
+
+
+def extrapolate(sample: dict, n_grid: int, n_krige: int) -> float:
+    """nodes/s of the full step mix from per-method sample rates."""
+    full = {"bilinear": n_grid, "spline": n_grid, "kriging": n_krige}
+    secs = sum(full[m] * sample[m][0] / sample[m][1] for m in full)
+    return (2 * n_grid + n_krige) / secs
+
+
+def cpu_baseline(name: str, budget_s: float = 20.0) -> dict:
+    import oracle
+    gw, sw, _ = make_inputs(name, 0)
+    cores = oracle.num_threads()
+    # sized for ~10-30 s of CPU work: kriging nodes scale with the thread count
+    kn = int(max(2000, min(sw.geom_out.n, budget_s * 0.6 * cores * 2.0e4 * (32.0 / sw.k) ** 3)))
+    smp = oracle_sample_step(name, gw, sw, krige_nodes=kn, grid_n_in=2048)
+    return {"value": extrapolate(smp, gw.geom_out.n, sw.geom_out.n), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": (f"float64 oracle, OpenMP x{cores}: bilinear+spline on the {min(2048, gw.geom_in.nx)}^2 crop of the input "
+                       f"({smp['bilinear'][1]} nodes each), kriging at {smp['kriging'][1]} evenly spaced nodes with the full "
+                       f"sounding set; per-method rates extrapolated to the step's node mix"),
+            "per_method_nodes_per_s": {m: smp[m][1] / smp[m][0] for m in smp}}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    gw, sw, _ = make_inputs(args.workload, 0)
+    cores = oracle.num_threads()
+    kn = int(max(1000, min(sw.geom_out.n, 4.0 * cores * 2.0e4 * (32.0 / sw.k) ** 3)))
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample_step(args.workload, gw, sw, krige_nodes=kn // 4, grid_n_in=512)
+    t0 = time.perf_counter()
+    vals = []
+    for _ in range(args.steps):
+        smp = oracle_sample_step(args.workload, gw, sw, krige_nodes=kn, grid_n_in=1024)
+        vals.append(extrapolate(smp, gw.geom_out.n, sw.geom_out.n))
+    dt = time.perf_counter() - t0
+    value = float(np.mean(vals))
+    sample = (f"per step: float64 oracle, OpenMP x{cores}, bilinear+spline on the 1024^2 crop ({smp['bilinear'][1]} nodes each), "
+              f"kriging at {smp['kriging'][1]} evenly spaced nodes with the full sounding set; rates extrapolated to the step's node mix")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.workload]["label"], "note": "ms_per_step is the wall time of one SAMPLE step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="default", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle work in cpu_baseline")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3                              # timing rule: W >= 3
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
