@@ -150,6 +150,15 @@ BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, i
                grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
                void* cuda_stream);
 
+/* Selects the implementation interp_spline uses (process-wide; for tests and profiling):
+ * 0 = automatic (default): the fused single-pass tile kernel where it applies (up-sampling, input at
+ *     least one solve window wide), else the global-solve path;
+ * 1 = fused tile kernel only (BATHY_ERR_GEOMETRY where it does not apply);
+ * 2 = global-solve path only (three batched full-length Thomas solves + gather evaluate).
+ * Both compute the same natural bicubic spline; DESIGN.md "Spline window bound" gives the bound on
+ * their difference (2.2e-7 x depth range). */
+BATHY_API int bathy_set_spline_path(int path);
+
 /* Static, never NULL. */
 BATHY_API const char* bathy_strerror(int status);
 

@@ -23,7 +23,7 @@ MAX_K = 64
 
 SYMBOLS = ["interp_bilinear", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
            "krige_predict", "krige_free_index", "krige_index_info", "interp_bilinear_host",
-           "interp_spline_host", "krige_host", "bathy_strerror", "bathy_launch_count"]
+           "interp_spline_host", "krige_host", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path"]
 
 
 class GridGeom(C.Structure):
@@ -69,6 +69,7 @@ def lib():
         L.bathy_strerror.argtypes = [C.c_int]
         L.bathy_strerror.restype = C.c_char_p
         L.bathy_launch_count.restype = C.c_int64
+        L.bathy_set_spline_path.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -98,6 +99,11 @@ def _dev_f32(t: torch.Tensor, name: str) -> torch.Tensor:
 
 def launch_count() -> int:
     return int(lib().bathy_launch_count())
+
+
+def set_spline_path(path: int) -> None:
+    """0 = automatic, 1 = fused tile kernel only, 2 = global-solve path only (include/bathy.h)."""
+    _check(lib().bathy_set_spline_path(int(path)), "bathy_set_spline_path")
 
 
 def interp_bilinear(z: torch.Tensor, gin, gout, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:

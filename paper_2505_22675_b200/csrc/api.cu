@@ -7,13 +7,14 @@ namespace bathy {
 
 int launch_bilinear(const float*, const grid_geom_t&, float*, const grid_geom_t&, cudaStream_t);
 size_t spline_workspace_bytes(const grid_geom_t&, const grid_geom_t&);
-int launch_spline(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t);
+int launch_spline(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t, int path);
 int build_index(const float*, const float*, const float*, int64_t, float, cudaStream_t, krige_index**);
 void free_index(krige_index*);
 int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, int, float*, int32_t*, int64_t*,
                    cudaStream_t);
 
 static std::atomic<int64_t> g_launches{0};
+static std::atomic<int> g_spline_path{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 static int check_variogram(const variogram_t& v)
@@ -65,7 +66,7 @@ BATHY_API int interp_spline(const float* d_in, grid_geom_t in, float* d_out, gri
     if (rc) return rc;
     if (!d_workspace || workspace_bytes < spline_workspace_bytes(in, out)) return BATHY_ERR_WORKSPACE;
     if (reinterpret_cast<uintptr_t>(d_workspace) % 256 != 0) return BATHY_ERR_WORKSPACE;
-    return launch_spline(d_in, in, d_out, out, d_workspace, static_cast<cudaStream_t>(cuda_stream));
+    return launch_spline(d_in, in, d_out, out, d_workspace, static_cast<cudaStream_t>(cuda_stream), g_spline_path.load());
 }
 
 BATHY_API int krige_build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n,
@@ -135,7 +136,7 @@ BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out
     DevBuf din(s), dout(s), ws(s);
     if (din.alloc(nin) || dout.alloc(nout) || ws.alloc(spline_workspace_bytes(in, out))) return BATHY_ERR_CUDA;
     BATHY_CUDA_TRY(cudaMemcpyAsync(din.p, h_in, nin, cudaMemcpyHostToDevice, s));
-    rc = launch_spline(static_cast<const float*>(din.p), in, static_cast<float*>(dout.p), out, ws.p, s);
+    rc = launch_spline(static_cast<const float*>(din.p), in, static_cast<float*>(dout.p), out, ws.p, s, g_spline_path.load());
     if (rc) return rc;
     BATHY_CUDA_TRY(cudaMemcpyAsync(h_out, dout.p, nout, cudaMemcpyDeviceToHost, s));
     BATHY_CUDA_TRY(cudaStreamSynchronize(s));
@@ -192,6 +193,13 @@ BATHY_API const char* bathy_strerror(int status)
         case BATHY_ERR_INDEX:     return "invalid kriging index handle";
         default:                  return "unknown status";
     }
+}
+
+BATHY_API int bathy_set_spline_path(int path)
+{
+    if (path < 0 || path > 2) return BATHY_ERR_GEOMETRY;
+    g_spline_path.store(path);
+    return BATHY_OK;
 }
 
 BATHY_API int64_t bathy_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }

@@ -1,14 +1,16 @@
 // bilinear.cu -- interp_bilinear (formula at L132).
 //
-// HBM-bound: the output write stream is 80-94 % of the bytes.  One CTA owns a TW x TH output tile.
-// It stages the covering input tile (+1 sample halo) in shared memory, minus a tile reference
-// depth z_ref so that the fp32 arithmetic runs on small numbers (|z| ~ 5000 m, ulp 4.9e-4 m), and
-// every thread marches down TH output rows for CPT columns that are lane-contiguous (column =
-// tile_x0 + e*THREADS + tid), so that every store instruction of a warp writes 128 contiguous
-// bytes whatever the alignment of the output row (nx_out = 8191 and 4093 are odd, so rows are not
-// 16-byte aligned and float4 stores would need a per-row shift that breaks the row-to-row reuse).
-// The horizontal interpolants H(j, column) are computed once per input row and reused for all
-// output rows that fall between input rows j and j+1.
+// HBM-bound (the output write stream is 80-94 % of the bytes) -- and, at ~1e12 nodes/s, issue-bound
+// unless a node costs fewer than ~10 instructions.  One CTA owns a TW x TH output tile.  It stages
+// the covering input tile (+1 sample halo) in shared memory, minus a tile reference depth z_ref so
+// that the fp32 arithmetic runs on small numbers (|z| ~ 5000 m, ulp 4.9e-4 m).  A thread owns CPT
+// columns that are lane-contiguous inside its warp (column = tile_x0 + warp*32*CPT + e*32 + lane),
+// so every store instruction of a warp writes 128 contiguous bytes whatever the alignment of the
+// output row (nx_out = 8191 and 4093 are odd: rows are not 16-byte aligned, and a per-row shift to
+// float4 alignment would break the row-to-row register reuse below).  The thread marches down the TH
+// rows: the horizontal interpolants of the two bracketing input rows live in registers and are
+// recomputed only when the output row enters a new input interval, so a node costs one FMA, one
+// add and one store plus its share of the per-row and per-interval work.
 #include "common.cuh"
 
 namespace bathy {
@@ -19,93 +21,97 @@ constexpr int kThreads = 256;
 
 template <int CPT, int TH>
 __global__ void __launch_bounds__(kThreads)
-bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out,
-                      AxisMap ax, AxisMap ay, int fw_cap, int fh_cap)
+bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay)
 {
     constexpr int TW = CPT * kThreads;
     extern __shared__ float s_tile[];                 // [fh][fw] input samples minus z_ref
-    __shared__ int   s_rowj[TH];                      // input row of each output row (-1: outside)
-    __shared__ float s_rows[TH];                      // local coordinate s of each output row
+    __shared__ int2  s_row[TH];                       // (input row j or -1, float bits of s) per output row
     __shared__ int   s_bounds[4];                     // i_lo, i_hi, j_lo, j_hi (sample indices)
 
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int J0 = blockIdx.x * TW;
     const int I0 = blockIdx.y * TH;
     const int Jlast = min(J0 + TW, ax.n_out) - 1;
     const int Ilast = min(I0 + TH, ay.n_out) - 1;
+    const int nrows = Ilast - I0 + 1;
 
     if (tid == 0) s_bounds[0] = axis_clamped(ax, J0);
     if (tid == 1) s_bounds[1] = axis_clamped(ax, Jlast) + 1;
     if (tid == 2) s_bounds[2] = axis_clamped(ay, I0);
     if (tid == 3) s_bounds[3] = axis_clamped(ay, Ilast) + 1;
     if (tid >= 32 && tid < 32 + TH) {
-        float s;
-        int r = tid - 32;
-        int j = (I0 + r <= Ilast) ? axis_locate(ay, I0 + r, &s) : -1;
-        s_rowj[r] = j;
-        s_rows[r] = (j < 0) ? 0.0f : s;
+        float s = 0.0f;
+        const int r = tid - 32;
+        const int j = (r < nrows) ? axis_locate(ay, I0 + r, &s) : -1;
+        s_row[r] = make_int2(j, __float_as_int(j < 0 ? 0.0f : s));
     }
-    // this thread's columns
+    // this thread's columns: interval index and local coordinate
+    const int Jt = J0 + warp * (32 * CPT) + lane;     // column of e = 0
     int   ci[CPT];
     float ct[CPT];
 #pragma unroll
     for (int e = 0; e < CPT; ++e) {
-        int J = J0 + e * kThreads + tid;
+        const int J = Jt + 32 * e;
+        ct[e] = 0.0f;
         ci[e] = (J <= Jlast) ? axis_locate(ax, J, &ct[e]) : -1;
-        if (ci[e] < 0) ct[e] = 0.0f;
     }
     __syncthreads();
     const int i_lo = s_bounds[0], i_hi = s_bounds[1], j_lo = s_bounds[2], j_hi = s_bounds[3];
     const int fw = i_hi - i_lo + 1, fh = j_hi - j_lo + 1;
-    (void)fw_cap; (void)fh_cap;
 
     float zref = __ldg(in + (size_t)j_lo * ax.n_in + i_lo);
     if (!isfinite(zref)) zref = 0.0f;
-    {
-        const int warp = tid >> 5, lane = tid & 31;
-        for (int r = warp; r < fh; r += kThreads / 32) {
-            const float* src = in + (size_t)(j_lo + r) * ax.n_in + i_lo;
-            float* dst = s_tile + r * fw;
-            for (int c = lane; c < fw; c += 32) dst[c] = __ldg(src + c) - zref;
-        }
+    for (int r = warp; r < fh; r += kThreads / 32) {
+        const float* __restrict__ src = in + (size_t)(j_lo + r) * ax.n_in + i_lo;
+        float* dst = s_tile + r * fw;
+#pragma unroll 4
+        for (int c = lane; c < fw; c += 32) dst[c] = __ldg(src + c) - zref;
     }
     __syncthreads();
 
-#pragma unroll
-    for (int e = 0; e < CPT; ++e) ci[e] = (ci[e] < 0) ? -1 : ci[e] - i_lo;
-
-    float hlo[CPT], hhi[CPT];
-#pragma unroll
-    for (int e = 0; e < CPT; ++e) hlo[e] = hhi[e] = 0.0f;
-    int cur_j = -2;
     const float qnan = __int_as_float(0x7fc00000);
-    for (int r = 0; r < TH; ++r) {
-        const int I = I0 + r;
-        if (I > Ilast) break;
-        const int j = s_rowj[r];
-        const float s = s_rows[r];
-        if (j >= 0 && j != cur_j) {                    // CTA-uniform branch: a new input row pair
+    bool cok[CPT];                                    // column is inside the tile (store predicate)
+    float cnan[CPT];                                  // NaN for a column outside the input extent, else 0
+    int   cofs[CPT];                                  // offset of the interval's left sample in a tile row
+#pragma unroll
+    for (int e = 0; e < CPT; ++e) {
+        cok[e] = (Jt + 32 * e) <= Jlast;
+        cnan[e] = (ci[e] < 0) ? qnan : 0.0f;
+        cofs[e] = max(ci[e] - i_lo, 0);
+    }
+
+    float hlo[CPT], hd[CPT];                          // lower interpolant and (upper - lower), relative to z_ref
+    float hhi[CPT];
+#pragma unroll
+    for (int e = 0; e < CPT; ++e) hlo[e] = hd[e] = hhi[e] = 0.0f;
+    int cur_j = -2;
+    float* orow = out + (size_t)I0 * ax.n_out + Jt;
+    for (int r = 0; r < nrows; ++r, orow += ax.n_out) {
+        const int2 rw = s_row[r];
+        const int j = rw.x;
+        const float s = __int_as_float(rw.y);
+        if (j < 0) {                                   // CTA-uniform: row outside the input extent
+#pragma unroll
+            for (int e = 0; e < CPT; ++e) if (cok[e]) orow[32 * e] = qnan;
+            continue;
+        }
+        if (j != cur_j) {                              // CTA-uniform: a new input row pair
             const float* row0 = s_tile + (j - j_lo) * fw;
             const float* row1 = row0 + fw;
             const bool step = (j == cur_j + 1);        // the old upper row is the new lower row
 #pragma unroll
             for (int e = 0; e < CPT; ++e) {
-                const int c = max(ci[e], 0);
-                hlo[e] = step ? hhi[e] : fmaf(ct[e], row0[c + 1] - row0[c], row0[c]);
+                const int c = cofs[e];
+                const float lo = step ? hhi[e] : fmaf(ct[e], row0[c + 1] - row0[c], row0[c]);
                 hhi[e] = fmaf(ct[e], row1[c + 1] - row1[c], row1[c]);
+                hd[e] = hhi[e] - lo;
+                hlo[e] = lo + cnan[e];
             }
             cur_j = j;
         }
-        float* orow = out + (size_t)I * ax.n_out;
 #pragma unroll
-        for (int e = 0; e < CPT; ++e) {
-            const int J = J0 + e * kThreads + tid;
-            if (J <= Jlast) {
-                float f = fmaf(s, hhi[e] - hlo[e], hlo[e]) + zref;
-                if (ci[e] < 0 || j < 0) f = qnan;
-                orow[J] = f;
-            }
-        }
+        for (int e = 0; e < CPT; ++e)
+            if (cok[e]) orow[32 * e] = fmaf(s, hd[e], hlo[e]) + zref;
     }
 }
 
@@ -138,7 +144,7 @@ int launch_bilinear(const float* d_in, const grid_geom_t& in, float* d_out, cons
                     cudaStream_t stream)
 {
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
-    constexpr int CPT = 2, TH = 16, TW = CPT * kThreads;
+    constexpr int CPT = 4, TH = 32, TW = CPT * kThreads;
     const long long fw = footprint_bound(ax, TW), fh = footprint_bound(ay, TH);
     const long long smem = fw * fh * (long long)sizeof(float);
     if (smem <= 160 * 1024 && (out.ny + TH - 1) / TH <= 65535) {
@@ -149,7 +155,7 @@ int launch_bilinear(const float* d_in, const grid_geom_t& in, float* d_out, cons
             attr_set = true;
         }
         dim3 grid((out.nx + TW - 1) / TW, (out.ny + TH - 1) / TH);
-        bilinear_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay, (int)fw, (int)fh);
+        bilinear_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay);
     } else {
         dim3 grid((out.nx + kThreads - 1) / kThreads, out.ny < 65535 ? out.ny : 65535);
         bilinear_gather_kernel<<<grid, kThreads, 0, stream>>>(d_in, d_out, ax, ay);

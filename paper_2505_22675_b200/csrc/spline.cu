@@ -100,9 +100,16 @@ size_t spline_workspace_bytes(const grid_geom_t& in, const grid_geom_t& /*out*/)
     return 3 * one;
 }
 
+int launch_spline_tiled(const float*, const grid_geom_t&, float*, const grid_geom_t&, cudaStream_t);   // spline_tile.cu
+
 int launch_spline(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
-                  void* d_ws, cudaStream_t stream)
+                  void* d_ws, cudaStream_t stream, int path)
 {
+    if (path != 2) {                                   // 0 = automatic, 1 = fused tiles only, 2 = global solves only
+        const int rc = launch_spline_tiled(d_in, in, d_out, out, stream);
+        if (rc != 1) return rc;
+        if (path == 1) return BATHY_ERR_GEOMETRY;
+    }
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
     const size_t n = (size_t)in.nx * (size_t)in.ny;
     const size_t one = (n * sizeof(float) + 255) / 256 * 256;

@@ -142,3 +142,63 @@ def test_host_forms_match_device_forms():
         dev = _run(method, w.z, w.geom_in, w.geom_out)
         host = hostfn(w.z, w.geom_in, w.geom_out)
         assert np.array_equal(dev, host)
+
+
+# ---------------------------------------------------------------------------------- spline paths
+# interp_spline has two implementations (include/bathy.h, bathy_set_spline_path): the fused tile
+# kernel (windowed Thomas solves) and the global-solve path.
+
+@pytest.fixture
+def spline_path():
+    b = _bathy()
+    yield b.set_spline_path
+    b.set_spline_path(0)
+
+
+@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("n_in,factor", [(89, 2), (57, 4), (90, 3), (130, 2), (41, 4), (193, 1)])
+def test_spline_both_paths_match_oracle(spline_path, path, n_in, factor):
+    # sizes at and just above one solve window, tiles with a single cell in the last row/column
+    w = W.grid_config(2, n_in=n_in, factor=factor, n_features=12, seed=500 + n_in)
+    ref = _ref("spline", w.z, w.geom_in, w.geom_out)
+    spline_path(path)
+    got = _run("spline", w.z, w.geom_in, w.geom_out)
+    err = max_abs_err(got, ref)
+    assert err <= TOL * depth_range(ref), (path, err, depth_range(ref))
+
+
+def test_spline_fused_rectangular_shifted_noninteger(spline_path):
+    rng = np.random.default_rng(77)
+    z = rng.normal(-4200, 25, (150, 260)).astype(np.float32)
+    gi = W.Geom(260, 150, 100.0, -50.0, 2.0, 3.0)
+    go = W.Geom(1500, 700, 95.0, -57.0, 0.353, 0.671)            # out-of-extent nodes on all four sides
+    ref = _ref("spline", z, gi, go)
+    assert np.isnan(ref).any()
+    for path in (1, 2):
+        spline_path(path)
+        got = _run("spline", z, gi, go)
+        assert max_abs_err(got, ref) <= TOL * depth_range(ref), path
+
+
+def test_spline_fused_worst_case_data(spline_path):
+    # white noise and a checkerboard: the largest second derivatives a given depth range allows,
+    # i.e. the worst case of the window bound
+    rng = np.random.default_rng(78)
+    ii, jj = np.meshgrid(np.arange(200), np.arange(300), indexing="ij")
+    for z in (rng.uniform(-6000, -5000, (200, 300)), -5500.0 + 500.0 * ((ii + jj) % 2)):
+        z = z.astype(np.float32)
+        gi, go = W.Geom(300, 200, 0, 0, 1, 1), W.Geom(1197, 797, 0, 0, 0.25, 0.25)
+        ref = _ref("spline", z, gi, go)
+        spline_path(1)
+        got = _run("spline", z, gi, go)
+        assert max_abs_err(got, ref) <= TOL * depth_range(ref)
+
+
+def test_spline_fused_path_refuses_what_it_cannot_serve(spline_path):
+    b = _bathy()
+    spline_path(1)
+    z = torch.zeros((20, 20), device="cuda")
+    with pytest.raises(b.BathyError):                             # smaller than a solve window
+        b.interp_spline(z, W.Geom(20, 20, 0, 0, 1, 1), W.Geom(39, 39, 0, 0, .5, .5))
+    spline_path(0)
+    b.interp_spline(z, W.Geom(20, 20, 0, 0, 1, 1), W.Geom(39, 39, 0, 0, .5, .5))   # automatic: global path
