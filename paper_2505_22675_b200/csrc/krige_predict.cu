@@ -1,18 +1,29 @@
 // krige_predict.cu -- ordinary kriging at every node of the output grid (
 // SURVEY.md 8(a) rows K2-K5).
 //
-// One warp walks a strip of consecutive nodes of one output row.
-//   K2  search: the warp collects, from the uniform cell grid, every sounding whose fp32 key
-//       (squared distance, the defined expression of reading K2) is <= an upper bound of the k-th
-//       key, then finds the exact k-th (key, index) by bisection on the key bits (ties: bisection
-//       on the index) with warp vote/reduce counts.  The bound for the next node of the strip is
-//       (r_k + node spacing)^2 by the triangle inequality, so only a thin annulus is ever in doubt.
+// One warp owns a BW x BH = 8 x 4 block of output nodes, lane l <-> node (l % 8, l / 8).
+//   K2  search, in two levels:
+//       pilot    the warp finds a key bound T such that at least k soundings lie within sqrt(T) of the
+//                block centre c (cell-grid scan + bisection on the key bits).  By the triangle
+//                inequality the k-th key of node q is then at most hi_q = (sqrt(T) + |q - c|)^2.
+//       gather   every sounding closer than sqrt(T) + max|q - c| to the block rectangle is copied once
+//                into shared memory (the candidate list all 32 nodes share; ~5 soundings per node).
+//       select   ONE THREAD PER NODE: pass 1 histograms the fp32 keys (reading K2: the defined
+//                expression) of the shared candidates into 32 buckets that are uniform in key over
+//                [0, hi_q] (private column of a shared-memory histogram); a scan finds the bucket b*
+//                that holds the k-th key; pass 2 takes every candidate below b* and lists the few in
+//                b*, among which the (key, index) ranking picks the rest -- exact, ties by index.
+//                No cross-lane traffic: a node's selection costs ~1/32 warp instruction per thread
+//                instruction, instead of a warp-wide bisection per node.
+//       A candidate list that does not fit splits the block into half blocks (down to single nodes).
 //   K3-K5 solve: G lanes per node (32/G nodes per warp at once), rows of C dealt cyclically to the
 //       lanes and held in REGISTERS (fully unrolled right-looking Cholesky); column j of L is
-//       published through a small shared-memory buffer and read back as broadcast float4.  The
-//       three right-hand sides c0, 1 and z ride along as forward substitutions, and
+//       published through a double-buffered shared-memory column and read back as broadcast float4.
+//       The three right-hand sides c0, 1 and z ride along as forward substitutions, and
 //           z_hat = y_z.y_c - mu * (y_z.y_1),   mu = (y_1.y_c - 1) / (y_1.y_1),   y_b = L^-1 b
 //       gives the Lagrange/Schur step without any back substitution or explicit weights.
+//       Covariances are built from coordinates relative to the block centre, pre-scaled by
+//       log2(e)/a (exponential) or 1/a (spherical): 7 / 10 instructions a pair.
 //   Tensor cores are not used: the factorisation is a k x k problem with a serial pivot chain.
 #include "krige_index.cuh"
 
@@ -22,6 +33,10 @@ namespace {
 
 constexpr int kWarpsPerCta = 4;
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int BW = 8, BH = 4;                    // node block of a warp
+constexpr int kBuckets = 32;                     // key histogram of the per-node selection
+constexpr int kCrit = 16;                        // listed candidates of the critical bucket
+constexpr float kPivEps = 1e-6f;                 // smallest accepted Cholesky pivot (sill = 1)
 
 struct PredictParams {
     const float4* pts;
@@ -32,23 +47,25 @@ struct PredictParams {
     float x0, y0, dx, dy;
     int k;
     float cpn;          // (sill - nugget) / sill : partial sill of the covariance normalised to sill = 1
-    float inv_range;    // 1 / a
-    float exp_scale;    // -log2(e) / a
-    float r0;           // first search radius of a strip
+    float lc;           // log2(cpn)                                   (exponential)
+    float c05, c15;     // 0.5 cpn, -1.5 cpn                           (spherical)
+    float s_coord;      // coordinate scale of the solve: log2(e)/a (exponential), 1/a (spherical)
+    float r0;           // first pilot radius
     float rmax;         // radius that certainly covers every sounding from any node of this call
     float* zhat;
     int32_t* nbr;
     unsigned long long* failed;
-    int strip_len, strips_per_row;
-    long long n_strips;
+    int nbx, nby;       // blocks per row / column of blocks
+    int chain;          // consecutive blocks walked by one warp
+    long long n_blocks;
 };
 
 template <int K, int G>
 struct Shape {
     static constexpr int R = K / G;             // rows of C per lane
     static constexpr int NB = 32 / G;           // nodes solved by a warp at once
-    static constexpr int CMAX = (4 * K > 128) ? 4 * K : 128;   // candidate buffer
-    static constexpr int NQ = CMAX / 32;
+    static constexpr int CAP = (K <= 32) ? 256 : 512;          // shared candidate list
+    static constexpr int NQ = CAP / 32;
     static constexpr int XYS = K + 4;           // float2 stride of a node's coordinate list (bank skew)
     static constexpr int CBS = K + 4;           // float stride of a node's column buffer (bank skew)
 };
@@ -56,14 +73,16 @@ struct Shape {
 template <int K, int G>
 struct __align__(16) WarpSmem {
     using S = Shape<K, G>;
-    float4   rhs[S::NB];                        // y_c, y_1, y_z of the current column, per node
-    float    colbuf[S::NB][S::CBS];             // column j of L, per node
-    float2   nb_xy[S::NB][S::XYS];              // neighbour coordinates
+    float4   rhs[2][S::NB];                     // -(y_c, y_1, y_z) of the current column, per node
+    float    colbuf[2][S::NB][S::CBS];          // -(column j of L), per node (double buffered)
+    float2   nb_xy[S::NB][S::XYS];              // neighbour coordinates, scaled, relative to the block centre
     float    nb_z[S::NB][K];                    // neighbour depths
-    int32_t  nb_idx[S::NB][K];                  // neighbour original indices
-    uint32_t cand_key[S::CMAX];
-    int32_t  cand_idx[S::CMAX];
-    int32_t  cand_pos[S::CMAX];
+    float2   cxy[S::CAP];                       // candidates: coordinates as given (fp32)
+    float    cz[S::CAP];                        //             depth (pilot: key bits)
+    int32_t  cid[S::CAP];                       //             original index
+    uint32_t hist[kBuckets + 1][32];            // per-lane key histogram (column = lane)
+    uint16_t nbl[K][32];                        // per-lane neighbour list: candidate slots
+    uint16_t crit[kCrit][32];                   // per-lane candidates of the critical bucket
 };
 
 // Reading K2: key = fmaf(ddx, ddx, ddy*ddy) in fp32, ddx = xq - x_i, ddy = yq - y_i.
@@ -73,34 +92,50 @@ __device__ __forceinline__ float knn_key(float xq, float yq, float x, float y)
     return __fmaf_rn(ddx, ddx, __fmul_rn(ddy, ddy));
 }
 
-// Covariance normalised to sill = 1: C(h) = 1 - gamma(h)/sill.  gamma(0) = 0 -> C(0) = 1.
-template <int MODEL>
-__device__ __forceinline__ float cov_of_h2(float h2, const PredictParams& p)
+__device__ __forceinline__ float rsqrt_approx(float v)
 {
-    const float h = h2 * rsqrtf(h2);                       // NaN at h2 == 0, replaced below
-    float c;
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+    return r;
+}
+
+__device__ __forceinline__ float ex2_approx(float v)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+    return r;
+}
+
+// Covariance normalised to sill = 1 from the squared distance in SCALED coordinates (h2 > 0):
+// exponential C = cpn exp(-h/a) = 2^(log2 cpn - h log2(e)/a) (no factor 3);
+// spherical   C = cpn (1 - 1.5 q + 0.5 q^3), q = min(h/a, 1).  h2 == 0 gives NaN (0 * inf): two
+// soundings at one place make the system singular and the node fails (reading K-dup).
+template <int MODEL>
+__device__ __forceinline__ float cov_scaled(float h2, const PredictParams& p)
+{
+    const float rs = rsqrt_approx(h2);
     if (MODEL == BATHY_VGM_EXPONENTIAL) {
-        c = p.cpn * exp2f(h * p.exp_scale);                // exp(-h/a), no factor 3
+        return ex2_approx(fmaf(-h2, rs, p.lc));
     } else {
-        const float q = h * p.inv_range;
-        c = (q < 1.0f) ? p.cpn * fmaf(q, fmaf(0.5f * q, q, -1.5f), 1.0f) : 0.0f;
+        float q;
+        asm("min.NaN.f32 %0, %1, %2;" : "=f"(q) : "f"(h2 * rs), "f"(1.0f));   // NaN (h2 == 0) survives
+        return fmaf(q, fmaf(q * q, p.c05, p.c15), p.cpn);
     }
-    return (h2 > 0.0f) ? c : 1.0f;
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2: collect every sounding with key bits <= key_hi inside the square of half-width r around the
-// node into the warp's candidate buffer, in index (cell-scan) order.  Returns the number found
-// (it may exceed CMAX, in which case the buffer is incomplete).
-template <int K, int G>
-__device__ __forceinline__ int collect(const PredictParams& p, WarpSmem<K, G>& ws, int lane,
-                                       float xq, float yq, float r, uint32_t key_hi)
+// Cell-grid scan: calls f(in_range, pt, n_so_far) for every sounding of the cells that overlap
+// [xlo, xhi] x [ylo, yhi], 32 soundings at a time (one per lane); f returns the keep predicate and
+// the scan compacts the kept ones: store(slot, pt) is called with consecutive slots.  Returns the
+// number kept (it may exceed `cap`, in which case the stores beyond cap were skipped).
+template <class Keep, class Store>
+__device__ __forceinline__ int scan_cells(const PredictParams& p, int lane, float xlo, float xhi, float ylo, float yhi,
+                                          int cap, Keep keep_fn, Store store_fn)
 {
-    using S = Shape<K, G>;
-    const float rs = r + 2e-3f * p.cell;                   // cell_of() rounding slack
-    const int cx0 = cell_of(xq - rs, p.xmin, p.inv_cell, p.ncx), cx1 = cell_of(xq + rs, p.xmin, p.inv_cell, p.ncx);
-    const int cy0 = cell_of(yq - rs, p.ymin, p.inv_cell, p.ncy), cy1 = cell_of(yq + rs, p.ymin, p.inv_cell, p.ncy);
-    int n_c = 0;
+    const float slack = 2e-3f * p.cell;                    // cell_of() rounding slack
+    const int cx0 = cell_of(xlo - slack, p.xmin, p.inv_cell, p.ncx), cx1 = cell_of(xhi + slack, p.xmin, p.inv_cell, p.ncx);
+    const int cy0 = cell_of(ylo - slack, p.ymin, p.inv_cell, p.ncy), cy1 = cell_of(yhi + slack, p.ymin, p.inv_cell, p.ncy);
+    int n = 0;
     for (int cyb = cy0; cyb <= cy1; cyb += 32) {
         const int cy = cyb + lane;
         int seg_s = 0, seg_e = 0;
@@ -113,138 +148,192 @@ __device__ __forceinline__ int collect(const PredictParams& p, WarpSmem<K, G>& w
             const int s = __shfl_sync(kFull, seg_s, rr), e = __shfl_sync(kFull, seg_e, rr);
             for (int base = s; base < e; base += 32) {
                 const int pos = base + lane;
+                float4 pt = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
                 bool keep = false;
-                uint32_t kb = 0;
-                int32_t id = 0;
                 if (pos < e) {
-                    const float4 pt = __ldg(p.pts + pos);
-                    kb = __float_as_uint(knn_key(xq, yq, pt.x, pt.y));
-                    id = __float_as_int(pt.w);
-                    keep = kb <= key_hi;
+                    pt = __ldg(p.pts + pos);
+                    keep = keep_fn(pt);
                 }
                 const unsigned m = __ballot_sync(kFull, keep);
-                const int off = n_c + __popc(m & ((1u << lane) - 1u));
-                if (keep && off < S::CMAX) {
-                    ws.cand_key[off] = kb;
-                    ws.cand_idx[off] = id;
-                    ws.cand_pos[off] = pos;
-                }
-                n_c += __popc(m);
+                const int off = n + __popc(m & ((1u << lane) - 1u));
+                if (keep && off < cap) store_fn(off, pt);
+                n += __popc(m);
             }
         }
     }
-    return n_c;
+    return n;
 }
 
-// K2: exact selection of the k smallest (key, index) among the n_c buffered candidates and
-// transfer of their (x, y, z, index) into neighbour slot `slot`.  Returns the k-th key bits
-// through *kth_key.  lo_hint: a value believed to satisfy count(key < lo_hint) < k (0 = none).
+// K2 pilot: a key bound T with at least k soundings within sqrt(T) of (cx, cy) and not many more.
+// `r` is the radius to try first and returns the radius that worked.  Returns a negative value for
+// degenerate input (more than CAP soundings at one distance).
 template <int K, int G>
-__device__ __forceinline__ void select_k(const PredictParams& p, WarpSmem<K, G>& ws, int lane, int slot,
-                                         int n_c, uint32_t lo_hint, uint32_t key_hi, uint32_t* kth_key)
+__device__ __forceinline__ float pilot(const PredictParams& p, WarpSmem<K, G>& ws, int lane, float cx, float cy, float& r)
 {
     using S = Shape<K, G>;
     const int k = p.k;
+    uint32_t* keys = reinterpret_cast<uint32_t*>(ws.cz);
+    float r_low = 0.0f, r_high = INFINITY;
+    int n = 0;
+    uint32_t key_hi = 0;
+    bool found = false;
+    for (int it = 0; it < 96; ++it) {
+        key_hi = __float_as_uint(fminf(r * r * 1.00001f, 3.0e38f));
+        n = scan_cells(p, lane, cx - r, cx + r, cy - r, cy + r, S::CAP,
+                       [&](const float4& pt) { return __float_as_uint(knn_key(cx, cy, pt.x, pt.y)) <= key_hi; },
+                       [&](int slot, const float4& pt) { keys[slot] = __float_as_uint(knn_key(cx, cy, pt.x, pt.y)); });
+        if (n < k) {
+            if (r >= p.rmax) break;                        // cannot happen for k <= n
+            r_low = r;
+            r = isinf(r_high) ? fminf(r * 1.5f, p.rmax) : 0.5f * (r_low + r_high);
+        } else if (n > S::CAP) {
+            r_high = r;
+            r = 0.5f * (r_low + r_high);
+        } else { found = true; break; }
+    }
+    __syncwarp();
+    if (!found) return -1.0f;
+    // tighten: bisection on the key bits until count(key <= hi) is in [k, k + k/4 + 2]
     uint32_t ck[S::NQ];
 #pragma unroll
     for (int q = 0; q < S::NQ; ++q) {
         const int c = lane + 32 * q;
-        ck[q] = (c < n_c) ? ws.cand_key[c] : 0xffffffffu;
+        ck[q] = (c < n) ? keys[c] : 0xffffffffu;
     }
-    auto count_le = [&](uint32_t v) {
+    uint32_t lo = 0, hi = key_hi;
+    int cnt_hi = n;
+    const int want = k + (k >> 2) + 2;
+    for (int step = 0; step < 16 && cnt_hi > want && lo < hi; ++step) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
         int c = 0;
 #pragma unroll
-        for (int q = 0; q < S::NQ; ++q) c += (ck[q] <= v) ? 1 : 0;
-        return (int)__reduce_add_sync(kFull, (unsigned)c);
-    };
-    uint32_t lo = lo_hint, hi = key_hi, tau = 0;
-    if (lo > 0 && count_le(lo - 1) >= k) lo = 0;           // the hint was not a lower bound
-    int cnt;
-    // invariant: count(key <= hi) >= k, count(key <= lo-1) < k
-    while (true) {
-        const uint32_t mid = lo + ((hi - lo) >> 1);
-        cnt = count_le(mid);
-        if (cnt == k) { tau = mid; break; }
-        if (cnt > k) hi = mid; else lo = mid + 1;
-        if (lo == hi) { tau = lo; cnt = count_le(tau); break; }
+        for (int q = 0; q < S::NQ; ++q) c += (ck[q] <= mid) ? 1 : 0;
+        c = (int)__reduce_add_sync(kFull, (unsigned)c);
+        if (c >= k) { hi = mid; cnt_hi = c; } else lo = mid + 1;
     }
-    int32_t idx_max = 0x7fffffff;                          // ties on the k-th key: lowest indices win
-    if (cnt != k) {
-        int32_t ci[S::NQ];
-        int below = 0;
-#pragma unroll
-        for (int q = 0; q < S::NQ; ++q) {
-            const int c = lane + 32 * q;
-            ci[q] = (c < n_c && ck[q] == tau) ? ws.cand_idx[c] : 0x7fffffff;   // 0x7fffffff is never a valid index (n <= 2^31-1)
-            below += (ck[q] < tau) ? 1 : 0;
-        }
-        const int want = k - (int)__reduce_add_sync(kFull, (unsigned)below);
-        int32_t ilo = 0, ihi = 0x7ffffffe;
-        while (true) {
-            const int32_t mid = ilo + ((ihi - ilo) >> 1);
-            int c = 0;
-#pragma unroll
-            for (int q = 0; q < S::NQ; ++q) c += (ci[q] <= mid) ? 1 : 0;
-            c = (int)__reduce_add_sync(kFull, (unsigned)c);
-            if (c == want) { idx_max = mid; break; }
-            if (c > want) ihi = mid; else ilo = mid + 1;
-            if (ilo == ihi) { idx_max = ilo; break; }
-        }
-    }
-    // transfer, preserving index (scan) order
-    int n_sel = 0;
-    uint32_t kmax = 0;
-#pragma unroll
-    for (int q = 0; q < S::NQ; ++q) {
-        if (32 * q < n_c) {                                // warp-uniform
-            const int c = lane + 32 * q;
-            bool sel = false;
-            int32_t id = 0;
-            if (c < n_c) {
-                id = ws.cand_idx[c];
-                sel = (ck[q] < tau) || (ck[q] == tau && id <= idx_max);
-            }
-            const unsigned m = __ballot_sync(kFull, sel);
-            const int off = n_sel + __popc(m & ((1u << lane) - 1u));
-            if (sel) {
-                const float4 pt = __ldg(p.pts + ws.cand_pos[c]);
-                ws.nb_xy[slot][off] = make_float2(pt.x, pt.y);
-                ws.nb_z[slot][off] = pt.z;
-                ws.nb_idx[slot][off] = id;
-                kmax = max(kmax, ck[q]);
-            }
-            n_sel += __popc(m);
-        }
-    }
-    *kth_key = __reduce_max_sync(kFull, kmax);
+    __syncwarp();
+    return __uint_as_float(hi);
 }
 
-// Parity/debug output: neighbours in ascending (key, index) order.
+// Bucket of a key in the per-lane histogram: round(key * scale) through the 1.5 * 2^23 magic
+// constant (no F2I).  Monotone non-decreasing in key, which is all the selection needs.
+__device__ __forceinline__ int bucket_of(float key, float scale)
+{
+    return __float_as_int(fmaf(key, scale, 12582912.0f)) - 0x4B400000;
+}
+
+// K2 select, one thread per node: the k candidates with the smallest (key, original index) among
+// the n_c shared candidates, all of them known to have key <= hi (hi < 0: lane idle).  Fills the
+// lane's column of ws.nbl with candidate slots.  Returns false if fewer than k candidates qualify
+// (cannot happen when hi is a valid bound).
 template <int K, int G>
-__device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSmem<K, G>& ws, int lane, int slot,
+__device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem<K, G>& ws, int lane, int n_c,
+                                                float xq, float yq, float hi)
+{
+    const int k = p.k;
+    const float scale = (float)kBuckets / fmaxf(hi, 1e-30f);
+#pragma unroll
+    for (int b = 0; b <= kBuckets; ++b) ws.hist[b][lane] = 0u;
+    // pass 1: histogram of the keys
+#pragma unroll 4
+    for (int c = 0; c < n_c; ++c) {
+        const float2 xy = ws.cxy[c];
+        const float key = knn_key(xq, yq, xy.x, xy.y);
+        if (key <= hi) ws.hist[bucket_of(key, scale)][lane] += 1u;
+    }
+    // the bucket that holds the k-th key
+    int bstar = kBuckets + 1, below = 0, cum = 0;
+#pragma unroll
+    for (int b = 0; b <= kBuckets; ++b) {
+        const int h = (int)ws.hist[b][lane];
+        if (bstar > kBuckets && cum + h >= k) { bstar = b; below = cum; }
+        cum += h;
+    }
+    if (hi < 0.0f) return true;
+    if (bstar > kBuckets) return false;
+    // pass 2: everything below the critical bucket is a neighbour; the critical bucket is listed
+    int cnt = 0, ncrit = 0;
+#pragma unroll 4
+    for (int c = 0; c < n_c; ++c) {
+        const float2 xy = ws.cxy[c];
+        const float key = knn_key(xq, yq, xy.x, xy.y);
+        if (key <= hi) {
+            const int b = bucket_of(key, scale);
+            if (b < bstar) { ws.nbl[cnt][lane] = (uint16_t)c; ++cnt; }
+            else if (b == bstar) { if (ncrit < kCrit) ws.crit[ncrit][lane] = (uint16_t)c; ++ncrit; }
+        }
+    }
+    const int need = k - below;                            // >= 1 candidates of the critical bucket
+    if (ncrit <= kCrit) {
+        for (int e = 0; e < ncrit; ++e) {                  // rank by (key, index) inside the bucket
+            const int ce = ws.crit[e][lane];
+            const float2 xe = ws.cxy[ce];
+            const uint32_t ke = __float_as_uint(knn_key(xq, yq, xe.x, xe.y));
+            const int32_t ie = ws.cid[ce];
+            int rank = 0;
+            for (int f = 0; f < ncrit; ++f) {
+                const int cf = ws.crit[f][lane];
+                const float2 xf = ws.cxy[cf];
+                const uint32_t kf = __float_as_uint(knn_key(xq, yq, xf.x, xf.y));
+                const int32_t jf = ws.cid[cf];
+                rank += (kf < ke || (kf == ke && jf < ie)) ? 1 : 0;
+            }
+            if (rank < need) { ws.nbl[cnt][lane] = (uint16_t)ce; ++cnt; }
+        }
+    } else {
+        // the list overflowed (many ties): take the `need` smallest (key, index) of the bucket one by one
+        uint32_t lk = 0; int32_t li = -1;                  // last taken
+        for (int t = 0; t < need; ++t) {
+            uint32_t bk = 0xffffffffu; int32_t bi = 0x7fffffff; int bc = -1;
+            for (int c = 0; c < n_c; ++c) {
+                const float2 xy = ws.cxy[c];
+                const float key = knn_key(xq, yq, xy.x, xy.y);
+                if (!(key <= hi) || bucket_of(key, scale) != bstar) continue;
+                const uint32_t kc = __float_as_uint(key);
+                const int32_t ic = ws.cid[c];
+                const bool after = (kc > lk) || (kc == lk && ic > li);
+                const bool better = (kc < bk) || (kc == bk && ic < bi);
+                if (after && better) { bk = kc; bi = ic; bc = c; }
+            }
+            if (bc < 0) return false;
+            ws.nbl[cnt][lane] = (uint16_t)bc; ++cnt;
+            lk = bk; li = bi;
+        }
+    }
+    return cnt == k;
+}
+
+// Parity/debug output, one thread per node: neighbours in ascending (key, index) order.
+template <int K, int G>
+__device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSmem<K, G>& ws, int lane,
                                                  float xq, float yq, long long node)
 {
     const int k = p.k;
-    for (int e = lane; e < k; e += 32) {
-        const float2 me = ws.nb_xy[slot][e];
-        const uint32_t mk = __float_as_uint(knn_key(xq, yq, me.x, me.y));
-        const int32_t mi = ws.nb_idx[slot][e];
+    for (int e = 0; e < k; ++e) {
+        const int ce = ws.nbl[e][lane];
+        const float2 xe = ws.cxy[ce];
+        const uint32_t ke = __float_as_uint(knn_key(xq, yq, xe.x, xe.y));
+        const int32_t ie = ws.cid[ce];
         int rank = 0;
         for (int f = 0; f < k; ++f) {
-            const float2 o = ws.nb_xy[slot][f];
-            const uint32_t ok = __float_as_uint(knn_key(xq, yq, o.x, o.y));
-            const int32_t oi = ws.nb_idx[slot][f];
-            rank += (ok < mk || (ok == mk && oi < mi)) ? 1 : 0;
+            const int cf = ws.nbl[f][lane];
+            const float2 xf = ws.cxy[cf];
+            const uint32_t kf = __float_as_uint(knn_key(xq, yq, xf.x, xf.y));
+            const int32_t jf = ws.cid[cf];
+            rank += (kf < ke || (kf == ke && jf < ie)) ? 1 : 0;
         }
-        p.nbr[node * k + rank] = mi;
+        p.nbr[node * k + rank] = ie;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// K3-K5 for the NB nodes whose neighbour lists sit in the warp's shared memory.
+// K3-K5 for the NB nodes whose neighbour lists (scaled coordinates relative to the block centre,
+// depths) sit in ws.nb_xy / ws.nb_z.  Lane (nd, g) = (lane / G, lane % G) holds rows g, g+G, ...
+// of node nd.  Rows at or beyond k are pad soundings placed far away from everything (covariance
+// exactly 0): they decouple as identity rows with zero right-hand sides.
 template <int K, int G, int MODEL>
-__device__ __forceinline__ void solve_nodes(const PredictParams& p, WarpSmem<K, G>& ws, int lane,
-                                            float xq, float yq, bool node_valid, long long node)
+__device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, G>& ws, int lane,
+                                            float xs, float ys, bool node_ok, long long node)
 {
     using S = Shape<K, G>;
     constexpr int R = S::R;
@@ -252,7 +341,7 @@ __device__ __forceinline__ void solve_nodes(const PredictParams& p, WarpSmem<K, 
     const int k = p.k;
     const float zref = ws.nb_z[nd][0];
 
-    float A[R][K];                   // A[t][m]: row g + G t, column m <= row (registers; only m < (t+1)G live)
+    float A[R][K];                   // A[t][m]: row g + G t, column m (only m < (t+1) G is live)
     float yc[R], y1[R], yz[R];
     float xr[R], yr[R];
 #pragma unroll
@@ -260,68 +349,69 @@ __device__ __forceinline__ void solve_nodes(const PredictParams& p, WarpSmem<K, 
         const int r = g + G * t;
         const float2 c = ws.nb_xy[nd][r];
         xr[t] = c.x; yr[t] = c.y;
-        const bool live = r < k;
-        const float ddx = xq - c.x, ddy = yq - c.y;
-        yc[t] = live ? cov_of_h2<MODEL>(fmaf(ddx, ddx, ddy * ddy), p) : 0.0f;
-        y1[t] = live ? 1.0f : 0.0f;
-        yz[t] = live ? ws.nb_z[nd][r] - zref : 0.0f;
+        const float ddx = xs - c.x, ddy = ys - c.y;
+        const float h2 = fmaf(ddx, ddx, ddy * ddy);
+        const float c0 = cov_scaled<MODEL>(h2, p);
+        yc[t] = (h2 > 0.0f) ? c0 : 1.0f;                   // gamma(0) = 0: a node on a datum sees the full sill
+        y1[t] = (r < k) ? 1.0f : 0.0f;
+        yz[t] = ws.nb_z[nd][r] - zref;
     }
-    // K3: lower triangle of C (rows beyond k are identity rows: they decouple and carry zero rhs)
+    // K3: block-lower triangle of C
 #pragma unroll
     for (int m = 0; m < K; ++m) {
         const float2 cm = ws.nb_xy[nd][m];
 #pragma unroll
         for (int t = m / G; t < R; ++t) {
-            const int r = g + G * t;
             const float ddx = xr[t] - cm.x, ddy = yr[t] - cm.y;
-            float c = cov_of_h2<MODEL>(fmaf(ddx, ddx, ddy * ddy), p);
-            if (r == m) c = 1.0f;
-            if (r >= k || m >= k) c = (r == m) ? 1.0f : 0.0f;
-            A[t][m] = c;
+            A[t][m] = cov_scaled<MODEL>(fmaf(ddx, ddx, ddy * ddy), p);
         }
+        if (g == m % G) A[m / G][m] = 1.0f;                // the diagonal: sill
     }
-    __syncwarp();
 
-    // K4: right-looking Cholesky, column by column; rhs vectors forward-substituted on the way
+    // K4: right-looking Cholesky, column by column; the three right-hand sides are forward-substituted
+    // on the way.  What is published (column of L, y_j) is NEGATED so that every update is a plain FMA.
     bool ok = true;
 #pragma unroll
     for (int j = 0; j < K; ++j) {
-        constexpr int dummy = 0; (void)dummy;
-        const int tj = j / G, gj = j % G;
+        const int tj = j / G, gj = j % G, buf = j & 1;
         const float piv = __shfl_sync(kFull, A[tj][j], gj, G);
-        ok = ok && (piv > 1e-6f);
-        const float inv = rsqrtf(piv);
+        ok = ok && (piv > kPivEps);
+        const float inv = rsqrt_approx(piv);
         float Lr[R];
 #pragma unroll
         for (int t = tj; t < R; ++t) {
-            const int r = g + G * t;
-            Lr[t] = (r > j) ? A[t][j] * inv : 0.0f;
-            ws.colbuf[nd][r] = Lr[t];
+            Lr[t] = A[t][j] * inv;
+            if (t == tj) Lr[t] = (g > gj) ? Lr[t] : 0.0f;  // rows <= j of the diagonal block are finished
+            ws.colbuf[buf][nd][g + G * t] = -Lr[t];
         }
-        if (g == gj) ws.rhs[nd] = make_float4(yc[tj] * inv, y1[tj] * inv, yz[tj] * inv, 0.0f);
+        {
+            const float a = yc[tj] * inv, b = y1[tj] * inv, c = yz[tj] * inv;
+            if (g == gj) {
+                yc[tj] = a; y1[tj] = b; yz[tj] = c;
+                ws.rhs[buf][nd] = make_float4(-a, -b, -c, 0.0f);
+            }
+        }
         __syncwarp();
-        const float4 yj = ws.rhs[nd];
+        const float4 yj = ws.rhs[buf][nd];
 #pragma unroll
         for (int t = tj; t < R; ++t) {
-            if (t == tj && g == gj) { yc[t] = yj.x; y1[t] = yj.y; yz[t] = yj.z; }
-            yc[t] = fmaf(-Lr[t], yj.x, yc[t]);
-            y1[t] = fmaf(-Lr[t], yj.y, y1[t]);
-            yz[t] = fmaf(-Lr[t], yj.z, yz[t]);
+            yc[t] = fmaf(Lr[t], yj.x, yc[t]);
+            y1[t] = fmaf(Lr[t], yj.y, y1[t]);
+            yz[t] = fmaf(Lr[t], yj.z, yz[t]);
         }
 #pragma unroll
         for (int m4 = (j + 1) / 4; m4 < K / 4; ++m4) {
-            const float4 L4 = *reinterpret_cast<const float4*>(&ws.colbuf[nd][4 * m4]);
+            const float4 L4 = *reinterpret_cast<const float4*>(&ws.colbuf[buf][nd][4 * m4]);
             const float Lm[4] = {L4.x, L4.y, L4.z, L4.w};
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const int m = 4 * m4 + e;
                 if (m > j) {
 #pragma unroll
-                    for (int t = (m / G > tj ? m / G : tj); t < R; ++t) A[t][m] = fmaf(-Lr[t], Lm[e], A[t][m]);
+                    for (int t = (m / G > tj ? m / G : tj); t < R; ++t) A[t][m] = fmaf(Lr[t], Lm[e], A[t][m]);
                 }
             }
         }
-        __syncwarp();
     }
 
     // K5 with the Schur step: four dot products over the G lanes of the node
@@ -340,7 +430,7 @@ __device__ __forceinline__ void solve_nodes(const PredictParams& p, WarpSmem<K, 
         d11 += __shfl_xor_sync(kFull, d11, o);
         d1z += __shfl_xor_sync(kFull, d1z, o);
     }
-    if (g == 0 && node_valid) {
+    if (g == 0 && node_ok) {
         const float mu = (d1c - 1.0f) / d11;
         float est = zref + (dcz - mu * d1z);
         if (!ok) {
@@ -356,90 +446,142 @@ __global__ void __launch_bounds__(kWarpsPerCta * 32)
 krige_predict_kernel(const PredictParams p)
 {
     using S = Shape<K, G>;
-    __shared__ WarpSmem<K, G> s_ws[kWarpsPerCta];
+    extern __shared__ __align__(16) unsigned char s_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    WarpSmem<K, G>& ws = s_ws[warp];
-    const long long sid = (long long)blockIdx.x * kWarpsPerCta + warp;
-    if (sid >= p.n_strips) return;
-    const int I = (int)(sid / p.strips_per_row);
-    const int Jbeg = (int)(sid % p.strips_per_row) * p.strip_len;
-    const int Jend = min(Jbeg + p.strip_len, p.nx);
-    const float yq = __fmaf_rn((float)I, p.dy, p.y0);
+    WarpSmem<K, G>& ws = reinterpret_cast<WarpSmem<K, G>*>(s_raw)[warp];
+    const long long wid = (long long)blockIdx.x * kWarpsPerCta + warp;
+    const long long b0 = wid * p.chain;
+    const long long b1 = min(b0 + (long long)p.chain, p.n_blocks);
     const int k = p.k;
+    const float qnan = __int_as_float(0x7fc00000);
+    float rho = p.r0;                                      // pilot radius to try first
 
-    float r = p.r0;                    // search radius to try
-    uint32_t lo_hint = 0;
-    float xprev = 0.0f;
-    bool have_prev = false;
-    float rk_prev = 0.0f;
+    for (long long blk = b0; blk < b1; ++blk) {
+        const int bj = (int)(blk % p.nbx), bi = (int)(blk / p.nbx);
+        const int J = bj * BW + (lane & (BW - 1)), I = bi * BH + (lane / BW);
+        const bool valid = (J < p.nx) && (I < p.ny);
+        const float xq = __fmaf_rn((float)J, p.dx, p.x0), yq = __fmaf_rn((float)I, p.dy, p.y0);
+        const long long node = (long long)I * p.nx + J;
 
-    for (int Jb = Jbeg; Jb < Jend; Jb += S::NB) {
-        float my_xq = 0.0f;            // node of this lane's group
-        bool my_valid = false;
-#pragma unroll 1
-        for (int s = 0; s < S::NB; ++s) {
-            const int J = Jb + s;
-            if (J >= Jend) break;                                   // warp-uniform
-            const float xq = __fmaf_rn((float)J, p.dx, p.x0);
-            if (lane / G == s) { my_xq = xq; my_valid = true; }
-            if (have_prev) {
-                const float step = fabsf(xq - xprev);
-                const float rhi = (rk_prev + step) * 1.00001f + 1e-30f;
-                const float rlo = fmaxf(rk_prev - step, 0.0f) * 0.99999f;
-                r = rhi;
-                lo_hint = __float_as_uint(rlo * rlo * 0.99999f);
-            }
-            float r_low = 0.0f, r_high = INFINITY;
+        int nsub = 1;                                      // the block is searched as nsub groups of 32/nsub lanes
+        for (int s = 0; s < nsub;) {
+            const int sz = 32 / nsub, l0 = s * sz;
+            int jx0, jx1, iy0, iy1;                        // the group's nodes inside the block
+            if (sz >= BW) { jx0 = 0; jx1 = BW - 1; iy0 = l0 / BW; iy1 = (l0 + sz - 1) / BW; }
+            else          { iy0 = iy1 = l0 / BW; jx0 = l0 % BW; jx1 = jx0 + sz - 1; }
+            const int Jlo = bj * BW + jx0, Jhi = min(bj * BW + jx1, p.nx - 1);
+            const int Ilo = bi * BH + iy0, Ihi = min(bi * BH + iy1, p.ny - 1);
+            if (Jlo > p.nx - 1 || Ilo > p.ny - 1) { ++s; continue; }       // no node of the grid in this group
+            const bool in_group = valid && lane >= l0 && lane < l0 + sz;
+            const float xlo = __fmaf_rn((float)Jlo, p.dx, p.x0), xhi = __fmaf_rn((float)Jhi, p.dx, p.x0);
+            const float ylo = __fmaf_rn((float)Ilo, p.dy, p.y0), yhi = __fmaf_rn((float)Ihi, p.dy, p.y0);
+            const float cx = 0.5f * (xlo + xhi), cy = 0.5f * (ylo + yhi);
+            // every bound below is inflated by far more than the fp32 rounding of the expressions in it
+            const float slack = 1e-6f * (fabsf(xlo) + fabsf(xhi) + fabsf(ylo) + fabsf(yhi)) + 1e-30f;
+            const float ex = 0.5f * (xhi - xlo) + slack, ey = 0.5f * (yhi - ylo) + slack;
+            const float dmax = sqrtf(ex * ex + ey * ey) * 1.00001f;
+
+            __syncwarp();
+            const float T = pilot<K, G>(p, ws, lane, cx, cy, rho);
+            bool group_ok = T >= 0.0f;
             int n_c = 0;
-            uint32_t key_hi = 0;
-            bool found = false;
-            for (int it = 0; it < 96; ++it) {
-                const float kh = r * r * 1.00001f;
-                key_hi = __float_as_uint(fminf(kh, 3.0e38f));
-                n_c = collect<K, G>(p, ws, lane, xq, yq, r, key_hi);
-                if (n_c < k) {
-                    if (r >= p.rmax) break;                         // cannot happen for k <= n
-                    r_low = r;
-                    r = isinf(r_high) ? fminf(r * 1.5f, p.rmax) : 0.5f * (r_low + r_high);
-                    lo_hint = 0;
-                } else if (n_c > S::CMAX) {
-                    r_high = r;
-                    r = 0.5f * (r_low + r_high);
-                } else { found = true; break; }
-            }
-            __syncwarp();
-            uint32_t kth = 0;
-            if (found) {
-                select_k<K, G>(p, ws, lane, s, n_c, lo_hint, key_hi, &kth);
+            float sT = 0.0f;
+            if (group_ok) {
+                sT = sqrtf(T) * 1.00001f;
+                rho = sT * 1.1f + slack;
+                const float Rb = (sT + dmax) * 1.0001f + slack;
+                const float Rb2 = Rb * Rb;
+                n_c = scan_cells(p, lane, cx - ex - Rb, cx + ex + Rb, cy - ey - Rb, cy + ey + Rb, S::CAP,
+                                 [&](const float4& pt) {
+                                     const float ax = fmaxf(fabsf(pt.x - cx) - ex, 0.0f), ay = fmaxf(fabsf(pt.y - cy) - ey, 0.0f);
+                                     return fmaf(ax, ax, ay * ay) <= Rb2;
+                                 },
+                                 [&](int slot, const float4& pt) {
+                                     ws.cxy[slot] = make_float2(pt.x, pt.y);
+                                     ws.cz[slot] = pt.z;
+                                     ws.cid[slot] = __float_as_int(pt.w);
+                                 });
+                __syncwarp();
+                if (n_c > S::CAP) {
+                    if (sz > 1) { nsub *= 2; s *= 2; continue; }           // split the group and search again
+                    group_ok = false;                                      // a single node: degenerate input
+                }
             } else {
-                // degenerate input (more than CMAX-k soundings at one distance): mark the node failed
-                for (int e = lane; e < K; e += 32) { ws.nb_xy[s][e] = make_float2(xq, yq); ws.nb_z[s][e] = 0.0f; ws.nb_idx[s][e] = -1; }
+                rho = p.r0;
             }
-            // pad the coordinate list so that the solve can read K entries
-            for (int e = k + lane; e < K; e += 32) { ws.nb_xy[s][e] = make_float2(0.0f, 0.0f); ws.nb_z[s][e] = 0.0f; ws.nb_idx[s][e] = -1; }
+            bool lane_ok = false;
+            if (group_ok) {
+                float hi = -1.0f;
+                if (in_group) {
+                    const float ddx = xq - cx, ddy = yq - cy;
+                    const float h = sT + (sqrtf(fmaf(ddx, ddx, ddy * ddy)) * 1.00001f + slack);
+                    hi = h * h * 1.00001f;
+                }
+                lane_ok = select_per_lane<K, G>(p, ws, lane, n_c, xq, yq, hi) && in_group;
+            }
+            if (in_group && !lane_ok) {                    // degenerate input: the node fails
+                p.zhat[node] = qnan;
+                if (p.failed) atomicAdd(p.failed, 1ull);
+            }
             __syncwarp();
-            if (p.nbr && found) write_sorted_nbr<K, G>(p, ws, lane, s, xq, yq, (long long)I * p.nx + J);
-            rk_prev = sqrtf(__uint_as_float(kth));
-            have_prev = found;
-            xprev = xq;
-            if (!found) { r = p.r0; lo_hint = 0; }
+            if (p.nbr && lane_ok) write_sorted_nbr<K, G>(p, ws, lane, xq, yq, node);
+
+            // K3-K5, NB nodes at a time
+            const unsigned solvable = __ballot_sync(kFull, lane_ok);
+            const float sc = p.s_coord;
+            const float padbase = 2.0f * (ex + ey + (sT + dmax) * 1.0001f + slack) * sc + 300.0f;
+            for (int bb = l0 / S::NB; bb * S::NB < l0 + sz; ++bb) {
+                if (((solvable >> (bb * S::NB)) & ((S::NB == 32) ? 0xffffffffu : ((1u << S::NB) - 1u))) == 0u) continue;
+                for (int e = lane; e < S::NB * K; e += 32) {
+                    const int nd = e / K, m = e % K, sl = bb * S::NB + nd;
+                    const bool node_live = (solvable >> sl) & 1u;
+                    float2 xy = make_float2(padbase + 300.0f * (float)m, 0.0f);
+                    float z = 0.0f;
+                    if (node_live) {
+                        const int c = ws.nbl[m < k ? m : 0][sl];
+                        z = ws.cz[c];
+                        if (m < k) {
+                            const float2 o = ws.cxy[c];
+                            xy = make_float2(__fmul_rn(o.x - cx, sc), __fmul_rn(o.y - cy, sc));
+                        }
+                    }
+                    ws.nb_xy[nd][m] = xy;
+                    ws.nb_z[nd][m] = z;
+                }
+                __syncwarp();
+                const int src = bb * S::NB + lane / G;     // the lane whose node this lane helps to solve
+                const int Js = bj * BW + (src & (BW - 1)), Is = bi * BH + (src / BW);
+                // __fmul_rn: no contraction into the subtractions of the solve, so that a node on a
+                // datum sees h2 == 0 exactly (same expression as the neighbour's coordinates)
+                const float xs = __fmul_rn(__fmaf_rn((float)Js, p.dx, p.x0) - cx, sc);
+                const float ys = __fmul_rn(__fmaf_rn((float)Is, p.dy, p.y0) - cy, sc);
+                solve_batch<K, G, MODEL>(p, ws, lane, xs, ys, (solvable >> src) & 1u, (long long)Is * p.nx + Js);
+                __syncwarp();
+            }
+            ++s;
         }
-        __syncwarp();
-        const int Jmine = Jb + lane / G;
-        solve_nodes<K, G, MODEL>(p, ws, lane, my_xq, yq, my_valid && Jmine < Jend, (long long)I * p.nx + Jmine);
-        __syncwarp();
     }
 }
 
 template <int K, int G>
 int launch_shape(const PredictParams& p, int model, cudaStream_t stream)
 {
-    const long long ctas = (p.n_strips + kWarpsPerCta - 1) / kWarpsPerCta;
+    const long long warps = (p.n_blocks + p.chain - 1) / p.chain;
+    const long long ctas = (warps + kWarpsPerCta - 1) / kWarpsPerCta;
     if (ctas > 0x7fffffffLL) return BATHY_ERR_SIZE;
+    const size_t smem = sizeof(WarpSmem<K, G>) * kWarpsPerCta;
+    static bool attr_set = false;
+    if (!attr_set) {
+        BATHY_CUDA_TRY(cudaFuncSetAttribute(krige_predict_kernel<K, G, BATHY_VGM_EXPONENTIAL>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        BATHY_CUDA_TRY(cudaFuncSetAttribute(krige_predict_kernel<K, G, BATHY_VGM_SPHERICAL>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
     if (model == BATHY_VGM_EXPONENTIAL)
-        krige_predict_kernel<K, G, BATHY_VGM_EXPONENTIAL><<<(unsigned)ctas, kWarpsPerCta * 32, 0, stream>>>(p);
+        krige_predict_kernel<K, G, BATHY_VGM_EXPONENTIAL><<<(unsigned)ctas, kWarpsPerCta * 32, smem, stream>>>(p);
     else
-        krige_predict_kernel<K, G, BATHY_VGM_SPHERICAL><<<(unsigned)ctas, kWarpsPerCta * 32, 0, stream>>>(p);
+        krige_predict_kernel<K, G, BATHY_VGM_SPHERICAL><<<(unsigned)ctas, kWarpsPerCta * 32, smem, stream>>>(p);
     count_launch();
     return launch_status();
 }
@@ -456,10 +598,14 @@ int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogr
     p.ncx = idx->ncx; p.ncy = idx->ncy;
     p.nx = out.nx; p.ny = out.ny; p.x0 = out.x0; p.y0 = out.y0; p.dx = out.dx; p.dy = out.dy;
     p.k = k;
-    p.cpn = (float)(((double)vg.sill - (double)vg.nugget) / (double)vg.sill);
-    p.inv_range = (float)(1.0 / (double)vg.range);
-    p.exp_scale = (float)(-1.4426950408889634 / (double)vg.range);
-    // first radius of a strip: the radius that holds ~1.5 k soundings at the mean density
+    const double cpn = ((double)vg.sill - (double)vg.nugget) / (double)vg.sill;
+    p.cpn = (float)cpn;
+    p.lc = cpn > 0.0 ? (float)log2(cpn) : -INFINITY;
+    p.c05 = (float)(0.5 * cpn);
+    p.c15 = (float)(-1.5 * cpn);
+    p.s_coord = (vg.model == BATHY_VGM_EXPONENTIAL) ? (float)(1.4426950408889634 / (double)vg.range)
+                                                    : (float)(1.0 / (double)vg.range);
+    // first pilot radius: the radius that holds ~1.5 k soundings at the mean density
     p.r0 = (float)((double)idx->step_hint * sqrt(1.5 * (double)k / 3.141592653589793));
     {
         // farthest any node of this call can be from any sounding: covers the union of both extents
@@ -474,13 +620,18 @@ int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogr
     p.zhat = d_zhat;
     p.nbr = d_nbr;
     p.failed = reinterpret_cast<unsigned long long*>(d_failed);
-    p.strip_len = 32;
-    p.strips_per_row = (out.nx + p.strip_len - 1) / p.strip_len;
-    p.n_strips = (long long)p.strips_per_row * out.ny;
+    p.nbx = (out.nx + BW - 1) / BW;
+    p.nby = (out.ny + BH - 1) / BH;
+    p.n_blocks = (long long)p.nbx * p.nby;
+    {
+        // blocks walked by one warp: enough CTAs for ~8 waves over the 148 SMs, at most 8 per warp
+        const long long per = p.n_blocks / ((long long)kSMs * 3 * kWarpsPerCta * 8);
+        p.chain = (int)(per < 1 ? 1 : (per > 8 ? 8 : per));
+    }
     if (k <= 8)  return launch_shape<8, 8>(p, vg.model, stream);
     if (k <= 16) return launch_shape<16, 8>(p, vg.model, stream);
     if (k <= 32) return launch_shape<32, 8>(p, vg.model, stream);
-    return launch_shape<64, 32>(p, vg.model, stream);
+    return launch_shape<64, 16>(p, vg.model, stream);
 }
 
 }  // namespace bathy
