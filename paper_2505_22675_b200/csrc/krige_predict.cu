@@ -327,22 +327,53 @@ __device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSme
 }
 
 // ---------------------------------------------------------------------------------------------
+// Packed fp32x2 arithmetic of sm_100 (FFMA2): one instruction, two FMAs -- half the issue slots of
+// the Cholesky trailing update.
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pack2(float lo, float hi)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float lo_of(u64 v)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+    return lo;
+}
+__device__ __forceinline__ float hi_of(u64 v)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+    return hi;
+}
+__device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c)
+{
+    u64 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+
 // K3-K5 for the NB nodes whose neighbour lists (scaled coordinates relative to the block centre,
 // depths) sit in ws.nb_xy / ws.nb_z.  Lane (nd, g) = (lane / G, lane % G) holds rows g, g+G, ...
-// of node nd.  Rows at or beyond k are pad soundings placed far away from everything (covariance
-// exactly 0): they decouple as identity rows with zero right-hand sides.
+// of node nd, two columns to a 64-bit register pair.  Rows at or beyond k are pad soundings placed
+// far away from everything (covariance exactly 0): they decouple as identity rows with zero
+// right-hand sides.
 template <int K, int G, int MODEL>
 __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, G>& ws, int lane,
                                             float xs, float ys, bool node_ok, long long node)
 {
     using S = Shape<K, G>;
     constexpr int R = S::R;
+    static_assert(G % 2 == 0 && K % 4 == 0, "column pairs must not straddle a row block");
     const int nd = lane / G, g = lane % G;
     const int k = p.k;
     const float zref = ws.nb_z[nd][0];
 
-    float A[R][K];                   // A[t][m]: row g + G t, column m (only m < (t+1) G is live)
-    float yc[R], y1[R], yz[R];
+    u64 A2[R][K / 2];                // A2[t][q] = (A[t][2q], A[t][2q+1]): row g + G t (only 2q < (t+1) G is live)
+    u64 yz1[R];                      // right-hand sides (z - z_ref, 1) of the row
+    float yc[R];                     // right-hand side c0 of the row
     float xr[R], yr[R];
 #pragma unroll
     for (int t = 0; t < R; ++t) {
@@ -353,87 +384,88 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
         const float h2 = fmaf(ddx, ddx, ddy * ddy);
         const float c0 = cov_scaled<MODEL>(h2, p);
         yc[t] = (h2 > 0.0f) ? c0 : 1.0f;                   // gamma(0) = 0: a node on a datum sees the full sill
-        y1[t] = (r < k) ? 1.0f : 0.0f;
-        yz[t] = ws.nb_z[nd][r] - zref;
+        yz1[t] = pack2(ws.nb_z[nd][r] - zref, (r < k) ? 1.0f : 0.0f);
     }
     // K3: block-lower triangle of C
 #pragma unroll
-    for (int m = 0; m < K; ++m) {
-        const float2 cm = ws.nb_xy[nd][m];
+    for (int q = 0; q < K / 2; ++q) {
+        const float4 cm = *reinterpret_cast<const float4*>(&ws.nb_xy[nd][2 * q]);     // (x, y) of columns 2q, 2q+1
 #pragma unroll
-        for (int t = m / G; t < R; ++t) {
-            const float ddx = xr[t] - cm.x, ddy = yr[t] - cm.y;
-            A[t][m] = cov_scaled<MODEL>(fmaf(ddx, ddx, ddy * ddy), p);
+        for (int t = (2 * q) / G; t < R; ++t) {
+            const float ax = xr[t] - cm.x, ay = yr[t] - cm.y, bx = xr[t] - cm.z, by = yr[t] - cm.w;
+            float ca = cov_scaled<MODEL>(fmaf(ax, ax, ay * ay), p);
+            float cb = cov_scaled<MODEL>(fmaf(bx, bx, by * by), p);
+            if (t == (2 * q) / G) {                        // the diagonal: sill
+                ca = (g == (2 * q) % G) ? 1.0f : ca;
+                cb = (g == (2 * q + 1) % G) ? 1.0f : cb;
+            }
+            A2[t][q] = pack2(ca, cb);
         }
-        if (g == m % G) A[m / G][m] = 1.0f;                // the diagonal: sill
     }
 
     // K4: right-looking Cholesky, column by column; the three right-hand sides are forward-substituted
-    // on the way.  What is published (column of L, y_j) is NEGATED so that every update is a plain FMA.
-    bool ok = true;
+    // on the way and their four dot products (the Schur step, K5) accumulate as the y_j appear.
+    // Row j's owner publishes P_j = (rhs_z, rhs_1, rhs_c, pivot) of its row -- final once column j-1
+    // has been applied, which it can do for its own row before anybody else has seen that column --
+    // in the same phase as column j-1 itself: one __syncwarp per column, no shuffles, and the rsqrt
+    // of the next pivot overlaps the trailing update.
+    float pmin = 1.0f;               // smallest pivot (a NaN pivot poisons every later column and the estimate)
+    u64 dots_c = pack2(0.0f, 0.0f);  // (y_c.y_z, y_c.y_1)
+    u64 dots_1 = pack2(0.0f, 0.0f);  // (y_1.y_z, y_1.y_1)
+    if (g == 0) ws.rhs[1][nd] = make_float4(lo_of(yz1[0]), hi_of(yz1[0]), yc[0], lo_of(A2[0][0]));
+    __syncwarp();
+    ulonglong2 P = *reinterpret_cast<const ulonglong2*>(&ws.rhs[1][nd]);
 #pragma unroll
     for (int j = 0; j < K; ++j) {
         const int tj = j / G, gj = j % G, buf = j & 1;
-        const float piv = __shfl_sync(kFull, A[tj][j], gj, G);
-        ok = ok && (piv > kPivEps);
+        const float piv = hi_of(P.y);
+        pmin = fminf(pmin, piv);
         const float inv = rsqrt_approx(piv);
-        float Lr[R];
+        const u64 yj = pack2(lo_of(P.x) * inv, hi_of(P.x) * inv);      // (y_z, y_1) of column j
+        const float ycj = lo_of(P.y) * inv, y1j = hi_of(yj);
+        dots_c = ffma2(pack2(ycj, ycj), yj, dots_c);
+        dots_1 = ffma2(pack2(y1j, y1j), yj, dots_1);
+        float nLr[R];
 #pragma unroll
         for (int t = tj; t < R; ++t) {
-            Lr[t] = A[t][j] * inv;
-            if (t == tj) Lr[t] = (g > gj) ? Lr[t] : 0.0f;  // rows <= j of the diagonal block are finished
-            ws.colbuf[buf][nd][g + G * t] = -Lr[t];
+            const float a = (j & 1) ? hi_of(A2[t][j / 2]) : lo_of(A2[t][j / 2]);
+            float sc = inv;
+            if (t == tj) sc = (g > gj) ? inv : 0.0f;       // rows <= j of the diagonal block are finished
+            const float l = a * sc;
+            ws.colbuf[buf][nd][g + G * t] = l;
+            nLr[t] = -l;
+            yz1[t] = ffma2(pack2(nLr[t], nLr[t]), yj, yz1[t]);
+            yc[t] = fmaf(nLr[t], ycj, yc[t]);
         }
-        {
-            const float a = yc[tj] * inv, b = y1[tj] * inv, c = yz[tj] * inv;
-            if (g == gj) {
-                yc[tj] = a; y1[tj] = b; yz[tj] = c;
-                ws.rhs[buf][nd] = make_float4(-a, -b, -c, 0.0f);
-            }
+        if (j + 1 < K) {                                   // P_{j+1}: row j+1 with column j applied
+            const int t1 = (j + 1) / G, g1 = (j + 1) % G;
+            const float a1 = ((j + 1) & 1) ? hi_of(A2[t1][(j + 1) / 2]) : lo_of(A2[t1][(j + 1) / 2]);
+            const float pv = fmaf(nLr[t1], -nLr[t1], a1);
+            if (g == g1) ws.rhs[buf][nd] = make_float4(lo_of(yz1[t1]), hi_of(yz1[t1]), yc[t1], pv);
         }
         __syncwarp();
-        const float4 yj = ws.rhs[buf][nd];
-#pragma unroll
-        for (int t = tj; t < R; ++t) {
-            yc[t] = fmaf(Lr[t], yj.x, yc[t]);
-            y1[t] = fmaf(Lr[t], yj.y, y1[t]);
-            yz[t] = fmaf(Lr[t], yj.z, yz[t]);
-        }
+        if (j + 1 < K) P = *reinterpret_cast<const ulonglong2*>(&ws.rhs[buf][nd]);
 #pragma unroll
         for (int m4 = (j + 1) / 4; m4 < K / 4; ++m4) {
-            const float4 L4 = *reinterpret_cast<const float4*>(&ws.colbuf[buf][nd][4 * m4]);
-            const float Lm[4] = {L4.x, L4.y, L4.z, L4.w};
+            const ulonglong2 L4 = *reinterpret_cast<const ulonglong2*>(&ws.colbuf[buf][nd][4 * m4]);
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int m = 4 * m4 + e;
-                if (m > j) {
+            for (int e = 0; e < 2; ++e) {
+                const int q = 2 * m4 + e;                  // columns 2q, 2q+1
+                if (2 * q + 1 > j) {
+                    const u64 Lq = e ? L4.y : L4.x;
 #pragma unroll
-                    for (int t = (m / G > tj ? m / G : tj); t < R; ++t) A[t][m] = fmaf(Lr[t], Lm[e], A[t][m]);
+                    for (int t = ((2 * q) / G > tj ? (2 * q) / G : tj); t < R; ++t)
+                        A2[t][q] = ffma2(pack2(nLr[t], nLr[t]), Lq, A2[t][q]);
                 }
             }
         }
     }
 
-    // K5 with the Schur step: four dot products over the G lanes of the node
-    float dcz = 0.0f, d1c = 0.0f, d11 = 0.0f, d1z = 0.0f;
-#pragma unroll
-    for (int t = 0; t < R; ++t) {
-        dcz = fmaf(yc[t], yz[t], dcz);
-        d1c = fmaf(y1[t], yc[t], d1c);
-        d11 = fmaf(y1[t], y1[t], d11);
-        d1z = fmaf(y1[t], yz[t], d1z);
-    }
-#pragma unroll
-    for (int o = G / 2; o > 0; o >>= 1) {
-        dcz += __shfl_xor_sync(kFull, dcz, o);
-        d1c += __shfl_xor_sync(kFull, d1c, o);
-        d11 += __shfl_xor_sync(kFull, d11, o);
-        d1z += __shfl_xor_sync(kFull, d1z, o);
-    }
     if (g == 0 && node_ok) {
+        const float dcz = lo_of(dots_c), d1c = hi_of(dots_c), d1z = lo_of(dots_1), d11 = hi_of(dots_1);
         const float mu = (d1c - 1.0f) / d11;
         float est = zref + (dcz - mu * d1z);
-        if (!ok) {
+        if (!(pmin > kPivEps) || !(est == est)) {
             est = __int_as_float(0x7fc00000);
             if (p.failed) atomicAdd(p.failed, 1ull);
         }
@@ -456,6 +488,7 @@ krige_predict_kernel(const PredictParams p)
     const float qnan = __int_as_float(0x7fc00000);
     float rho = p.r0;                                      // pilot radius to try first
 
+#pragma unroll 1
     for (long long blk = b0; blk < b1; ++blk) {
         const int bj = (int)(blk % p.nbx), bi = (int)(blk / p.nbx);
         const int J = bj * BW + (lane & (BW - 1)), I = bi * BH + (lane / BW);
@@ -464,6 +497,7 @@ krige_predict_kernel(const PredictParams p)
         const long long node = (long long)I * p.nx + J;
 
         int nsub = 1;                                      // the block is searched as nsub groups of 32/nsub lanes
+#pragma unroll 1
         for (int s = 0; s < nsub;) {
             const int sz = 32 / nsub, l0 = s * sz;
             int jx0, jx1, iy0, iy1;                        // the group's nodes inside the block
@@ -530,6 +564,7 @@ krige_predict_kernel(const PredictParams p)
             const unsigned solvable = __ballot_sync(kFull, lane_ok);
             const float sc = p.s_coord;
             const float padbase = 2.0f * (ex + ey + (sT + dmax) * 1.0001f + slack) * sc + 300.0f;
+#pragma unroll 1
             for (int bb = l0 / S::NB; bb * S::NB < l0 + sz; ++bb) {
                 if (((solvable >> (bb * S::NB)) & ((S::NB == 32) ? 0xffffffffu : ((1u << S::NB) - 1u))) == 0u) continue;
                 for (int e = lane; e < S::NB * K; e += 32) {
