@@ -31,7 +31,6 @@ namespace bathy {
 
 namespace {
 
-constexpr int kWarpsPerCta = 4;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int BW = 8, BH = 4;                    // node block of a warp
 constexpr int kBuckets = 32;                     // key histogram of the per-node selection
@@ -65,8 +64,9 @@ struct Shape {
     static constexpr int R = K / G;             // rows of C per lane
     static constexpr int NB = 32 / G;           // nodes solved by a warp at once
     static constexpr int CAP = (K <= 32) ? 256 : 512;          // shared candidate list
+    static constexpr int WARPS = (K <= 32) ? 16 : 8;           // warps per CTA: one CTA per SM (registers)
     static constexpr int NQ = CAP / 32;
-    static constexpr int XYS = K + 4;           // float2 stride of a node's coordinate list (bank skew)
+    static constexpr int XYS = K + 4;           // float stride of a node's coordinate lists (bank skew)
     static constexpr int CBS = K + 4;           // float stride of a node's column buffer (bank skew)
 };
 
@@ -75,12 +75,13 @@ struct __align__(16) WarpSmem {
     using S = Shape<K, G>;
     float4   rhs[2][S::NB];                     // -(y_c, y_1, y_z) of the current column, per node
     float    colbuf[2][S::NB][S::CBS];          // -(column j of L), per node (double buffered)
-    float2   nb_xy[S::NB][S::XYS];              // neighbour coordinates, scaled, relative to the block centre
+    float    nb_x[S::NB][S::XYS];               // neighbour coordinates, scaled, relative to the block centre
+    float    nb_y[S::NB][S::XYS];
     float    nb_z[S::NB][K];                    // neighbour depths
     float2   cxy[S::CAP];                       // candidates: coordinates as given (fp32)
     float    cz[S::CAP];                        //             depth (pilot: key bits)
     int32_t  cid[S::CAP];                       //             original index
-    uint32_t hist[kBuckets + 1][32];            // per-lane key histogram (column = lane)
+    uint16_t hist[kBuckets + 1][32];            // per-lane key histogram (column = lane)
     uint16_t nbl[K][32];                        // per-lane neighbour list: candidate slots
     uint16_t crit[kCrit][32];                   // per-lane candidates of the critical bucket
 };
@@ -193,24 +194,27 @@ __device__ __forceinline__ float pilot(const PredictParams& p, WarpSmem<K, G>& w
     }
     __syncwarp();
     if (!found) return -1.0f;
-    // tighten: bisection on the key bits until count(key <= hi) is in [k, k + k/4 + 2]
+    // tighten: T = the smallest value of a fixed grid (fp32 patterns whose low 16 bits are all ones:
+    // 0.8 % steps) with at least k keys at or below it.  It depends on the soundings and the centre
+    // only -- not on the radius the scan happened to use -- so a block gives the same candidate
+    // list, hence bit-identical depths, whatever call, tile or launch shape it is part of.
     uint32_t ck[S::NQ];
 #pragma unroll
     for (int q = 0; q < S::NQ; ++q) {
         const int c = lane + 32 * q;
         ck[q] = (c < n) ? keys[c] : 0xffffffffu;
     }
-    uint32_t lo = 0, hi = key_hi;
-    int cnt_hi = n;
-    const int want = k + (k >> 2) + 2;
-    for (int step = 0; step < 16 && cnt_hi > want && lo < hi; ++step) {
+    uint32_t lo = 0, hi = key_hi >> 16;
+    while (lo < hi) {
         const uint32_t mid = lo + ((hi - lo) >> 1);
+        const uint32_t v = (mid << 16) | 0xffffu;
         int c = 0;
 #pragma unroll
-        for (int q = 0; q < S::NQ; ++q) c += (ck[q] <= mid) ? 1 : 0;
+        for (int q = 0; q < S::NQ; ++q) c += (ck[q] <= v) ? 1 : 0;
         c = (int)__reduce_add_sync(kFull, (unsigned)c);
-        if (c >= k) { hi = mid; cnt_hi = c; } else lo = mid + 1;
+        if (c >= k) hi = mid; else lo = mid + 1;
     }
+    hi = (hi << 16) | 0xffffu;
     __syncwarp();
     return __uint_as_float(hi);
 }
@@ -233,13 +237,13 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     const int k = p.k;
     const float scale = (float)kBuckets / fmaxf(hi, 1e-30f);
 #pragma unroll
-    for (int b = 0; b <= kBuckets; ++b) ws.hist[b][lane] = 0u;
+    for (int b = 0; b <= kBuckets; ++b) ws.hist[b][lane] = (uint16_t)0;
     // pass 1: histogram of the keys
 #pragma unroll 4
     for (int c = 0; c < n_c; ++c) {
         const float2 xy = ws.cxy[c];
         const float key = knn_key(xq, yq, xy.x, xy.y);
-        if (key <= hi) ws.hist[bucket_of(key, scale)][lane] += 1u;
+        if (key <= hi) ws.hist[bucket_of(key, scale)][lane] += (uint16_t)1;
     }
     // the bucket that holds the k-th key
     int bstar = kBuckets + 1, below = 0, cum = 0;
@@ -355,8 +359,34 @@ __device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c)
     return d;
 }
 
+__device__ __forceinline__ u64 fmul2(u64 a, u64 b)
+{
+    u64 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// Two covariances at once (see cov_scaled): the distance and polynomial arithmetic is packed, the
+// two rsqrt and the two ex2 go to the MUFU pipe one by one.
+template <int MODEL>
+__device__ __forceinline__ u64 cov2_scaled(u64 h2, const PredictParams& p)
+{
+    const u64 rs2 = pack2(rsqrt_approx(lo_of(h2)), rsqrt_approx(hi_of(h2)));
+    const u64 q2 = fmul2(h2, rs2);                         // scaled distances
+    if (MODEL == BATHY_VGM_EXPONENTIAL) {
+        return pack2(ex2_approx(p.lc - lo_of(q2)), ex2_approx(p.lc - hi_of(q2)));
+    } else {
+        float qa, qb;
+        asm("min.NaN.f32 %0, %1, %2;" : "=f"(qa) : "f"(lo_of(q2)), "f"(1.0f));   // NaN (h2 == 0) survives
+        asm("min.NaN.f32 %0, %1, %2;" : "=f"(qb) : "f"(hi_of(q2)), "f"(1.0f));
+        const u64 q = pack2(qa, qb);
+        const u64 pp = ffma2(fmul2(q, q), pack2(p.c05, p.c05), pack2(p.c15, p.c15));
+        return ffma2(q, pp, pack2(p.cpn, p.cpn));
+    }
+}
+
 // K3-K5 for the NB nodes whose neighbour lists (scaled coordinates relative to the block centre,
-// depths) sit in ws.nb_xy / ws.nb_z.  Lane (nd, g) = (lane / G, lane % G) holds rows g, g+G, ...
+// depths) sit in ws.nb_x, ws.nb_y, ws.nb_z.  Lane (nd, g) = (lane / G, lane % G) holds rows g, g+G, ...
 // of node nd, two columns to a 64-bit register pair.  Rows at or beyond k are pad soundings placed
 // far away from everything (covariance exactly 0): they decouple as identity rows with zero
 // right-hand sides.
@@ -378,28 +408,30 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
 #pragma unroll
     for (int t = 0; t < R; ++t) {
         const int r = g + G * t;
-        const float2 c = ws.nb_xy[nd][r];
-        xr[t] = c.x; yr[t] = c.y;
-        const float ddx = xs - c.x, ddy = ys - c.y;
+        xr[t] = ws.nb_x[nd][r]; yr[t] = ws.nb_y[nd][r];
+        const float ddx = xs - xr[t], ddy = ys - yr[t];
         const float h2 = fmaf(ddx, ddx, ddy * ddy);
-        const float c0 = cov_scaled<MODEL>(h2, p);
+        const float c0 = lo_of(cov2_scaled<MODEL>(pack2(h2, h2), p));
         yc[t] = (h2 > 0.0f) ? c0 : 1.0f;                   // gamma(0) = 0: a node on a datum sees the full sill
         yz1[t] = pack2(ws.nb_z[nd][r] - zref, (r < k) ? 1.0f : 0.0f);
     }
-    // K3: block-lower triangle of C
+    // K3: block-lower triangle of C, two columns at a time in packed fp32x2 arithmetic
+    const u64 neg1 = pack2(-1.0f, -1.0f);
 #pragma unroll
     for (int q = 0; q < K / 2; ++q) {
-        const float4 cm = *reinterpret_cast<const float4*>(&ws.nb_xy[nd][2 * q]);     // (x, y) of columns 2q, 2q+1
+        const u64 cx2 = *reinterpret_cast<const u64*>(&ws.nb_x[nd][2 * q]);    // x of columns 2q, 2q+1
+        const u64 cy2 = *reinterpret_cast<const u64*>(&ws.nb_y[nd][2 * q]);
 #pragma unroll
         for (int t = (2 * q) / G; t < R; ++t) {
-            const float ax = xr[t] - cm.x, ay = yr[t] - cm.y, bx = xr[t] - cm.z, by = yr[t] - cm.w;
-            float ca = cov_scaled<MODEL>(fmaf(ax, ax, ay * ay), p);
-            float cb = cov_scaled<MODEL>(fmaf(bx, bx, by * by), p);
+            const u64 dx2 = ffma2(cx2, neg1, pack2(xr[t], xr[t]));
+            const u64 dy2 = ffma2(cy2, neg1, pack2(yr[t], yr[t]));
+            u64 c2 = cov2_scaled<MODEL>(ffma2(dx2, dx2, fmul2(dy2, dy2)), p);
             if (t == (2 * q) / G) {                        // the diagonal: sill
-                ca = (g == (2 * q) % G) ? 1.0f : ca;
-                cb = (g == (2 * q + 1) % G) ? 1.0f : cb;
+                const float ca = (g == (2 * q) % G) ? 1.0f : lo_of(c2);
+                const float cb = (g == (2 * q + 1) % G) ? 1.0f : hi_of(c2);
+                c2 = pack2(ca, cb);
             }
-            A2[t][q] = pack2(ca, cb);
+            A2[t][q] = c2;
         }
     }
 
@@ -474,14 +506,14 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
 }
 
 template <int K, int G, int MODEL>
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+__global__ void __launch_bounds__(Shape<K, G>::WARPS * 32, 1)
 krige_predict_kernel(const PredictParams p)
 {
     using S = Shape<K, G>;
     extern __shared__ __align__(16) unsigned char s_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     WarpSmem<K, G>& ws = reinterpret_cast<WarpSmem<K, G>*>(s_raw)[warp];
-    const long long wid = (long long)blockIdx.x * kWarpsPerCta + warp;
+    const long long wid = (long long)blockIdx.x * S::WARPS + warp;
     const long long b0 = wid * p.chain;
     const long long b1 = min(b0 + (long long)p.chain, p.n_blocks);
     const int k = p.k;
@@ -489,7 +521,12 @@ krige_predict_kernel(const PredictParams p)
     float rho = p.r0;                                      // pilot radius to try first
 
 #pragma unroll 1
-    for (long long blk = b0; blk < b1; ++blk) {
+    for (int it = 0; it < p.chain; ++it) {
+        const long long blk = b0 + it;
+        // One CTA barrier per block, between its search and its solves: the warps of the CTA then run
+        // the (long, fully unrolled) solve code side by side and share its instruction-cache lines.
+        bool synced = false;
+        if (blk >= b1) { __syncthreads(); continue; }
         const int bj = (int)(blk % p.nbx), bi = (int)(blk / p.nbx);
         const int J = bj * BW + (lane & (BW - 1)), I = bi * BH + (lane / BW);
         const bool valid = (J < p.nx) && (I < p.ny);
@@ -561,6 +598,7 @@ krige_predict_kernel(const PredictParams p)
             if (p.nbr && lane_ok) write_sorted_nbr<K, G>(p, ws, lane, xq, yq, node);
 
             // K3-K5, NB nodes at a time
+            if (!synced) { __syncthreads(); synced = true; }
             const unsigned solvable = __ballot_sync(kFull, lane_ok);
             const float sc = p.s_coord;
             const float padbase = 2.0f * (ex + ey + (sT + dmax) * 1.0001f + slack) * sc + 300.0f;
@@ -580,7 +618,8 @@ krige_predict_kernel(const PredictParams p)
                             xy = make_float2(__fmul_rn(o.x - cx, sc), __fmul_rn(o.y - cy, sc));
                         }
                     }
-                    ws.nb_xy[nd][m] = xy;
+                    ws.nb_x[nd][m] = xy.x;
+                    ws.nb_y[nd][m] = xy.y;
                     ws.nb_z[nd][m] = z;
                 }
                 __syncwarp();
@@ -595,6 +634,7 @@ krige_predict_kernel(const PredictParams p)
             }
             ++s;
         }
+        if (!synced) __syncthreads();
     }
 }
 
@@ -602,6 +642,7 @@ template <int K, int G>
 int launch_shape(const PredictParams& p, int model, cudaStream_t stream)
 {
     const long long warps = (p.n_blocks + p.chain - 1) / p.chain;
+    constexpr int kWarpsPerCta = Shape<K, G>::WARPS;
     const long long ctas = (warps + kWarpsPerCta - 1) / kWarpsPerCta;
     if (ctas > 0x7fffffffLL) return BATHY_ERR_SIZE;
     const size_t smem = sizeof(WarpSmem<K, G>) * kWarpsPerCta;
@@ -660,7 +701,7 @@ int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogr
     p.n_blocks = (long long)p.nbx * p.nby;
     {
         // blocks walked by one warp: enough CTAs for ~8 waves over the 148 SMs, at most 8 per warp
-        const long long per = p.n_blocks / ((long long)kSMs * 3 * kWarpsPerCta * 8);
+        const long long per = p.n_blocks / ((long long)kSMs * 16 * 8);
         p.chain = (int)(per < 1 ? 1 : (per > 8 ? 8 : per));
     }
     if (k <= 8)  return launch_shape<8, 8>(p, vg.model, stream);
