@@ -700,9 +700,11 @@ int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogr
     p.nby = (out.ny + BH - 1) / BH;
     p.n_blocks = (long long)p.nbx * p.nby;
     {
-        // blocks walked by one warp: enough CTAs for ~8 waves over the 148 SMs, at most 8 per warp
-        const long long per = p.n_blocks / ((long long)kSMs * 16 * 8);
-        p.chain = (int)(per < 1 ? 1 : (per > 8 ? 8 : per));
+        // one block per warp: the hardware CTA scheduler balances the uneven sounding density best
+        // (measured: 5.91 ms with 1 block per warp, 5.99 ms with 8, 6.80 ms with 16 on config 4);
+        // longer chains only where the grid would exceed the CTA-count limit
+        const long long per = p.n_blocks / (0x7fffffffLL / 2) + 1;
+        p.chain = (int)per;
     }
     if (k <= 8)  return launch_shape<8, 8>(p, vg.model, stream);
     if (k <= 16) return launch_shape<16, 8>(p, vg.model, stream);
