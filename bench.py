@@ -129,8 +129,9 @@ def make_inputs(name: str, rank: int):
     spec = WORKLOADS[name]
     gc, n_in, factor, nf = spec["grid"]
     kc, width, n_target, n_out = spec["krige"]
-    gw = W.grid_config(gc, n_in=n_in, factor=factor, n_features=nf, seed=W.SEEDS[gc] + 100 * rank)
-    sw = W.sounding_config(kc, width=width, n_target=n_target, n_out=n_out, seed=W.SEEDS[kc] + 100 * rank)
+    from paper_2505_22675_b200 import sharding as S
+    gw = W.grid_config(gc, n_in=n_in, factor=factor, n_features=nf, seed=S.rank_seed(W.SEEDS[gc], rank))
+    sw = W.sounding_config(kc, width=width, n_target=n_target, n_out=n_out, seed=S.rank_seed(W.SEEDS[kc], rank))
     if spec["tiles"]:
         tiles = W.boustrophedon_tiles(n_out, max(n_out // 8, 1))
     else:
@@ -219,10 +220,9 @@ def run_ours(args):
 
     seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])        # ms per segment
     total_ms = float(evs[0][0].elapsed_time(evs[-1][4]))
-    t = torch.tensor([total_ms] + seg.mean(axis=0).tolist(), dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, ms_bil, ms_spl, ms_idx, ms_krg = t.tolist()
+    from paper_2505_22675_b200 import sharding
+    total_ms, ms_bil, ms_spl, ms_idx, ms_krg = sharding.reduce_step_times(
+        [total_ms] + seg.mean(axis=0).tolist(), dist, dev)          # max over ranks
     ms_per_step = total_ms / args.steps
 
     # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the timed region)
@@ -246,10 +246,7 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_ms = (time.perf_counter() - te0) * 1e3 / e2e_steps
-    te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_ms = float(te.item())
+    e2e_ms = sharding.reduce_step_times([e2e_ms], dist, dev)[0]
     h2d = 2 * gi.n * 4 + 3 * sw.x.shape[0] * 4
     d2h = 2 * n_grid * 4 + n_krige * 4 + 8
 
