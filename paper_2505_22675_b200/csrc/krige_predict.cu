@@ -330,42 +330,6 @@ __device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSme
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// Packed fp32x2 arithmetic of sm_100 (FFMA2): one instruction, two FMAs -- half the issue slots of
-// the Cholesky trailing update.
-typedef unsigned long long u64;
-__device__ __forceinline__ u64 pack2(float lo, float hi)
-{
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ float lo_of(u64 v)
-{
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-    return lo;
-}
-__device__ __forceinline__ float hi_of(u64 v)
-{
-    float lo, hi;
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-    return hi;
-}
-__device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c)
-{
-    u64 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-
-__device__ __forceinline__ u64 fmul2(u64 a, u64 b)
-{
-    u64 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-
 // Two covariances at once (see cov_scaled): the distance and polynomial arithmetic is packed, the
 // two rsqrt and the two ex2 go to the MUFU pipe one by one.
 template <int MODEL>

@@ -93,29 +93,33 @@ spline_eval_kernel(const float* __restrict__ z, const float* __restrict__ Mx, co
 
 }  // namespace
 
-size_t spline_workspace_bytes(const grid_geom_t& in, const grid_geom_t& /*out*/)
+size_t spline_tiled_table_bytes(const grid_geom_t&, const grid_geom_t&);                                      // spline_tile.cu
+int launch_spline_tiled(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t);   // spline_tile.cu
+
+// Workspace: the axis tables of the fused path, then the three second-derivative planes of the
+// global-solve path.
+size_t spline_workspace_bytes(const grid_geom_t& in, const grid_geom_t& out)
 {
     const size_t n = (size_t)in.nx * (size_t)in.ny;
     const size_t one = (n * sizeof(float) + 255) / 256 * 256;
-    return 3 * one;
+    return spline_tiled_table_bytes(in, out) + 3 * one;
 }
-
-int launch_spline_tiled(const float*, const grid_geom_t&, float*, const grid_geom_t&, cudaStream_t);   // spline_tile.cu
 
 int launch_spline(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
                   void* d_ws, cudaStream_t stream, int path)
 {
     if (path != 2) {                                   // 0 = automatic, 1 = fused tiles only, 2 = global solves only
-        const int rc = launch_spline_tiled(d_in, in, d_out, out, stream);
+        const int rc = launch_spline_tiled(d_in, in, d_out, out, d_ws, stream);
         if (rc != 1) return rc;
         if (path == 1) return BATHY_ERR_GEOMETRY;
     }
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
     const size_t n = (size_t)in.nx * (size_t)in.ny;
     const size_t one = (n * sizeof(float) + 255) / 256 * 256;
-    float* Mx = reinterpret_cast<float*>(static_cast<char*>(d_ws));
-    float* My = reinterpret_cast<float*>(static_cast<char*>(d_ws) + one);
-    float* Mxy = reinterpret_cast<float*>(static_cast<char*>(d_ws) + 2 * one);
+    char* planes = static_cast<char*>(d_ws) + spline_tiled_table_bytes(in, out);
+    float* Mx = reinterpret_cast<float*>(planes);
+    float* My = reinterpret_cast<float*>(planes + one);
+    float* Mxy = reinterpret_cast<float*>(planes + 2 * one);
     const float hx = in.dx, hy = in.dy;
     const float six_hx2 = (float)(6.0 / ((double)hx * (double)hx)), six_hy2 = (float)(6.0 / ((double)hy * (double)hy));
     // S1: rows (along x): system = row, elements contiguous
