@@ -125,11 +125,20 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
             const float* row1 = row0 + pitch;
             const bool step = (j == cur_j + 1);        // the old upper row is the new lower row
             float lo[CPT];
+            if (step) {                                // (a real branch: the lower row is not read again)
+#pragma unroll
+                for (int e = 0; e < CPT; ++e) lo[e] = hhi[e];
+            } else {
+#pragma unroll
+                for (int e = 0; e < CPT; ++e) {
+                    const int c = cofs[e];
+                    lo[e] = fmaf(ct[e], row0[c + 1] - row0[c], row0[c] - zref);
+                }
+            }
+            // (sample - z_ref): the arithmetic runs on small numbers (|z| ~ 5000 m, ulp 4.9e-4 m)
 #pragma unroll
             for (int e = 0; e < CPT; ++e) {
                 const int c = cofs[e];
-                // (sample - z_ref): the arithmetic runs on small numbers (|z| ~ 5000 m, ulp 4.9e-4 m)
-                lo[e] = step ? hhi[e] : fmaf(ct[e], row0[c + 1] - row0[c], row0[c] - zref);
                 hhi[e] = fmaf(ct[e], row1[c + 1] - row1[c], row1[c] - zref);
             }
 #pragma unroll

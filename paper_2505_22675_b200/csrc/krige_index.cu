@@ -46,14 +46,23 @@ bbox_partial_kernel(const float* __restrict__ x, const float* __restrict__ y, in
 
 __global__ void bbox_final_kernel(const float4* __restrict__ partial, int nb, float4* __restrict__ out)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    float4 r = partial[0];
-    for (int b = 1; b < nb; ++b) {
+    // one warp: lanes stride over the partials, then a shuffle tree (min/max are order independent:
+    // deterministic)
+    float xmin = INFINITY, xmax = -INFINITY, ymin = INFINITY, ymax = -INFINITY;
+    bool bad = false;
+    for (int b = threadIdx.x; b < nb; b += 32) {
         const float4 p = partial[b];
-        r.x = (isnan(r.x) || isnan(p.x)) ? NAN : fminf(r.x, p.x);
-        r.y = fmaxf(r.y, p.y); r.z = fminf(r.z, p.z); r.w = fmaxf(r.w, p.w);
+        bad |= isnan(p.x);
+        xmin = fminf(xmin, p.x); xmax = fmaxf(xmax, p.y); ymin = fminf(ymin, p.z); ymax = fmaxf(ymax, p.w);
     }
-    *out = r;
+    for (int o = 16; o > 0; o >>= 1) {
+        xmin = fminf(xmin, __shfl_xor_sync(0xffffffffu, xmin, o));
+        xmax = fmaxf(xmax, __shfl_xor_sync(0xffffffffu, xmax, o));
+        ymin = fminf(ymin, __shfl_xor_sync(0xffffffffu, ymin, o));
+        ymax = fmaxf(ymax, __shfl_xor_sync(0xffffffffu, ymax, o));
+    }
+    bad = __any_sync(0xffffffffu, bad);
+    if (threadIdx.x == 0) *out = make_float4(bad ? NAN : xmin, xmax, ymin, ymax);
 }
 
 // ---- histogram of soundings per cell
