@@ -141,7 +141,7 @@ spline_tables_kernel(AxisMap ax, AxisMap ay, float4* __restrict__ coltab, float4
 }
 
 template <class S>
-__global__ void __launch_bounds__(kTileThreads)
+__global__ void __launch_bounds__(kTileThreads, 4)
 spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay,
                    const float4* __restrict__ coltab, const float4* __restrict__ rowtab,
                    const int* __restrict__ tbx, const int* __restrict__ tby, const int* __restrict__ rfirst,
@@ -170,14 +170,21 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const int ax0 = w0x & ~3, offx = w0x - ax0;
         float* dstz = s_zbuf + buf * (WY * PA);
         if (vec_ok) {
+            // a warp takes whole window rows, a lane one 16-byte vector of the row: everything that
+            // depends on the column is computed once, a row costs one address add and one cp.async
             constexpr int VPR = PA / 4;
-            for (int v = tid; v < WY * VPR; v += kTileThreads) {
-                const int r = v / VPR, c4 = (v - r * VPR) * 4;
-                const int col = ax0 + c4;
-                const int bytes = max(0, min(16, (ax.n_in - col) * 4));  // past the row end: zero fill
-                const float* src = in + (size_t)(w0y + r) * ax.n_in + min(col, ax.n_in - 4);
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(dstz + r * PA + c4);
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(bytes) : "memory");
+            static_assert(VPR <= 32, "a window row is at most 32 vectors");
+            const int col = ax0 + 4 * lane;
+            const int bytes = max(0, min(16, (ax.n_in - col) * 4));      // past the row end: zero fill
+            const float* src = in + (size_t)(w0y + warp) * ax.n_in + min(col, ax.n_in - 4);
+            unsigned dst = (unsigned)__cvta_generic_to_shared(dstz + warp * PA + 4 * lane);
+            if (lane < VPR) {
+#pragma unroll 4
+                for (int r = warp; r < WY; r += NW) {
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(bytes) : "memory");
+                    src += (size_t)NW * ax.n_in;
+                    dst += NW * PA * 4;
+                }
             }
         } else {
             for (int v = tid; v < WY * WX; v += kTileThreads) {
@@ -243,8 +250,9 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         //      packed FMAs for two columns.  The row loop of an interval has no data-dependent branch.
         const float qnan = __int_as_float(0x7fc00000);
         const u64 neg1 = pack2(-1.0f, -1.0f), zref2 = pack2(zref, zref);
-        if ((byt == 0 || (byt + 1) * TYI >= ay.n_in - 1) && Ibeg < Iend &&
-            (__float_as_int(__ldg(rowtab + Ibeg).x) < 0 || __float_as_int(__ldg(rowtab + Iend - 1).x) < 0)) {
+        const bool oob_rows = (byt == 0 || (byt + 1) * TYI >= ay.n_in - 1) && Ibeg < Iend &&
+            (__float_as_int(__ldg(rowtab + Ibeg).x) < 0 || __float_as_int(__ldg(rowtab + Iend - 1).x) < 0);
+        if (oob_rows) {
             // rows of the tile outside the input extent (reading B4): NaN
             for (int I = Ibeg + warp; I < Iend; I += NW)
                 if (__float_as_int(__ldg(rowtab + I).x) < 0)
@@ -288,6 +296,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
 #pragma unroll
             for (int p = 0; p < 2; ++p) X0[p] = X1[p] = Xd[p] = Y0[p] = Y1[p] = pack2(0.0f, 0.0f);
             const u64 cn2[2] = {pack2(cnan[0], cnan[1]), pack2(cnan[2], cnan[3])};
+            const bool full = !oob_rows && (Jp + 128 <= Jend);        // warp-uniform
             int curk = -2;
 #pragma unroll
             for (int ki = 0; ki < TI; ++ki) {
@@ -308,19 +317,36 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 }
                 curk = kj;
                 float* op = out + (size_t)rs * ax.n_out + Jt;
+                if (full) {                            // all four columns inside the tile, no row outside the extent
 #pragma unroll 2
-                for (int r = rs; r < re; ++r, op += ax.n_out) {
-                    const float4 rw = __ldg(rowtab + r);               // (j, s, Cy, Dy); j < 0: row outside the extent
-                    const bool rv = __float_as_int(rw.x) >= 0;
-                    const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
+                    for (int r = rs; r < re; ++r, op += ax.n_out) {
+                        const float4 rw = __ldg(rowtab + r);           // (j, s, Cy, Dy)
+                        const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
 #pragma unroll
-                    for (int p = 0; p < 2; ++p) {
-                        u64 o = ffma2(s2, Xd[p], X0[p]);
-                        o = ffma2(cy2, Y0[p], o);
-                        o = ffma2(dy2, Y1[p], o);
-                        o = fadd2(o, zref2);
-                        if (cok[2 * p] && rv) op[64 * p] = lo_of(o);
-                        if (cok[2 * p + 1] && rv) op[64 * p + 32] = hi_of(o);
+                        for (int p = 0; p < 2; ++p) {
+                            u64 o = ffma2(s2, Xd[p], X0[p]);
+                            o = ffma2(cy2, Y0[p], o);
+                            o = ffma2(dy2, Y1[p], o);
+                            o = fadd2(o, zref2);
+                            op[64 * p] = lo_of(o);
+                            op[64 * p + 32] = hi_of(o);
+                        }
+                    }
+                } else {
+#pragma unroll 1
+                    for (int r = rs; r < re; ++r, op += ax.n_out) {
+                        const float4 rw = __ldg(rowtab + r);           // (j, s, Cy, Dy); j < 0: row outside the extent
+                        const bool rv = __float_as_int(rw.x) >= 0;
+                        const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
+#pragma unroll
+                        for (int p = 0; p < 2; ++p) {
+                            u64 o = ffma2(s2, Xd[p], X0[p]);
+                            o = ffma2(cy2, Y0[p], o);
+                            o = ffma2(dy2, Y1[p], o);
+                            o = fadd2(o, zref2);
+                            if (cok[2 * p] && rv) op[64 * p] = lo_of(o);
+                            if (cok[2 * p + 1] && rv) op[64 * p + 32] = hi_of(o);
+                        }
                     }
                 }
             }
