@@ -233,13 +233,29 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
 
         // ---- S1: Mx' = Thomas along x of z on the knot rows (warp 0 -> Q.xy = (z, Mx'));
         //      S3: Mxy' = Thomas along x of My' (warp 1 -> Q.zw = (My', Mxy'))
-        if (warp < 2 && lane < nky) {
+        if (inner_x) {
+            // interior tile: every warp works -- plane = warp & 1 (z or My'), half = warp >> 1: the row's
+            // knots are solved as two overlapping windows of HW = TXI/2 + 1 + 2H knots (the same
+            // 0.268^H bound applies where the halves meet), so the serial chains are 55 instead of 87 long
+            constexpr int HL = TXI / 2 + 1;                               // knots kept by the left half
+            constexpr int HW = HL + 2 * H;                                // window of a half
+            if (lane < nky) {
+                const int plane = warp & 1, half = warp >> 1;
+                const float* row = (plane == 0 ? s_zf : s_my) + lane * PZ + (half ? WX - HW : 0);
+                float2* dst = reinterpret_cast<float2*>(s_q + lane * PQ + (half ? HL : 0)) + plane;
+                auto rd = [&](int q) { return row[q]; };
+                auto st = [&](int k, float v, float m) { dst[2 * k] = make_float2(v, m); };
+                // left: window knots [0, HW), kept = tile knots [0, HL) = window [H, H + HL)
+                // right: window knots [WX - HW, WX), kept = tile knots [HL, NXI) = window [HW - H - (NXI - HL), HW - H)
+                if (half == 0) thomas_window<HW, true, H, HL>(rd, st, 0, 0);
+                else           thomas_window<HW, true, HW - H - (NXI - HL), NXI - HL>(rd, st, 0, 0);
+            }
+        } else if (warp < 2 && lane < nky) {
             const float* row = (warp == 0 ? s_zf : s_my) + lane * PZ;
             float2* dst = reinterpret_cast<float2*>(s_q + lane * PQ) + warp;
             auto rd = [&](int q) { return row[q]; };
             auto st = [&](int k, float v, float m) { dst[2 * k] = make_float2(v, m); };
-            if (inner_x) thomas_window<WX, true, H, NXI>(rd, st, 0, 0);
-            else         thomas_window<WX, false, 0, 0>(rd, st, kx0, nkx);
+            thomas_window<WX, false, 0, 0>(rd, st, kx0, nkx);
         }
         __syncthreads();
 
