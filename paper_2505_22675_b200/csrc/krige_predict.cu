@@ -512,7 +512,8 @@ krige_predict_kernel(const PredictParams p)
             const float ylo = __fmaf_rn((float)Ilo, p.dy, p.y0), yhi = __fmaf_rn((float)Ihi, p.dy, p.y0);
             const float cx = 0.5f * (xlo + xhi), cy = 0.5f * (ylo + yhi);
             // every bound below is inflated by far more than the fp32 rounding of the expressions in it
-            const float slack = 1e-6f * (fabsf(xlo) + fabsf(xhi) + fabsf(ylo) + fabsf(yhi)) + 1e-30f;
+            // (4 ulp of the largest coordinate: centre, half extents and distances are each a few roundings)
+            const float slack = 5e-7f * fmaxf(fmaxf(fabsf(xlo), fabsf(xhi)), fmaxf(fabsf(ylo), fabsf(yhi))) + 1e-30f;
             const float ex = 0.5f * (xhi - xlo) + slack, ey = 0.5f * (yhi - ylo) + slack;
             const float dmax = sqrtf(ex * ex + ey * ey) * 1.00001f;
 
