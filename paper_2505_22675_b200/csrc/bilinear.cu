@@ -102,59 +102,71 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
 
     // Two columns to a 64-bit register pair: a node is half a packed FMA (FFMA2) and a store.
     u64 hlo2[CPT / 2], hd2[CPT / 2];                  // lower interpolant (+ z_ref) and (upper - lower)
-    float hhi[CPT];
-#pragma unroll
-    for (int e = 0; e < CPT; ++e) hhi[e] = 0.0f;
 #pragma unroll
     for (int p = 0; p < CPT / 2; ++p) hlo2[p] = hd2[p] = pack2(0.0f, 0.0f);
     int cur_j = -2;
     float* orow = out + (size_t)I0 * ax.n_out + Jt;
+    // interval change: the horizontal interpolants of input row `row` at this thread's columns, on
+    // (sample - z_ref) so that the arithmetic runs on small numbers (|z| ~ 5000 m, ulp 4.9e-4 m),
+    // two columns at a time in packed arithmetic
+    const u64 nzref2 = pack2(-zref, -zref), neg1 = pack2(-1.0f, -1.0f);
+    const u64 ct2[CPT / 2] = {pack2(ct[0], ct[1]), pack2(ct[2], ct[3])};
+    const u64 cz2[CPT / 2] = {pack2(cz[0], cz[1]), pack2(cz[2], cz[3])};
+    static_assert(CPT == 4, "column pairs are written out for CPT = 4");
+    auto hrow = [&](const float* row, u64* h2) {
+#pragma unroll
+        for (int p = 0; p < CPT / 2; ++p) {
+            const int c0 = cofs[2 * p], c1 = cofs[2 * p + 1];
+            const u64 l = pack2(row[c0], row[c1]), r = pack2(row[c0 + 1], row[c1 + 1]);
+            h2[p] = ffma2(ct2[p], ffma2(l, neg1, r), fadd2(l, nzref2));
+        }
+    };
+    u64 hhi2[CPT / 2] = {pack2(0.0f, 0.0f), pack2(0.0f, 0.0f)};
+    // interior tile (CTA-uniform): every column inside the tile, every row inside the input extent
+    const bool full = (J0 + TW - 1 <= Jlast) && s_row[0].x >= 0 && s_row[nrows - 1].x >= 0;
     int2 rw_next = s_row[0];
     for (int r = 0; r < nrows; ++r, orow += ax.n_out) {
         const int2 rw = rw_next;
         rw_next = s_row[min(r + 1, TH - 1)];          // the next row's entry is in flight while this row is stored
         const int j = rw.x;
         const float s = __int_as_float(rw.y);
-        if (j < 0) {                                   // CTA-uniform: row outside the input extent
+        if (!full && j < 0) {                          // CTA-uniform: row outside the input extent
 #pragma unroll
             for (int e = 0; e < CPT; ++e) if (cok[e]) orow[32 * e] = qnan;
             continue;
         }
         if (j != cur_j) {                              // CTA-uniform: a new input row pair
             const float* row0 = s_tile + (j - j_lo) * pitch;
-            const float* row1 = row0 + pitch;
-            const bool step = (j == cur_j + 1);        // the old upper row is the new lower row
-            float lo[CPT];
-            if (step) {                                // (a real branch: the lower row is not read again)
+            u64 lo2[CPT / 2];
+            if (j == cur_j + 1) {                      // the old upper row is the new lower row
 #pragma unroll
-                for (int e = 0; e < CPT; ++e) lo[e] = hhi[e];
+                for (int p = 0; p < CPT / 2; ++p) lo2[p] = hhi2[p];
             } else {
-#pragma unroll
-                for (int e = 0; e < CPT; ++e) {
-                    const int c = cofs[e];
-                    lo[e] = fmaf(ct[e], row0[c + 1] - row0[c], row0[c] - zref);
-                }
+                hrow(row0, lo2);
             }
-            // (sample - z_ref): the arithmetic runs on small numbers (|z| ~ 5000 m, ulp 4.9e-4 m)
-#pragma unroll
-            for (int e = 0; e < CPT; ++e) {
-                const int c = cofs[e];
-                hhi[e] = fmaf(ct[e], row1[c + 1] - row1[c], row1[c] - zref);
-            }
+            hrow(row0 + pitch, hhi2);
 #pragma unroll
             for (int p = 0; p < CPT / 2; ++p) {
-                const u64 l2 = pack2(lo[2 * p], lo[2 * p + 1]);
-                hd2[p] = ffma2(l2, pack2(-1.0f, -1.0f), pack2(hhi[2 * p], hhi[2 * p + 1]));
-                hlo2[p] = fadd2(l2, pack2(cz[2 * p], cz[2 * p + 1]));
+                hd2[p] = ffma2(lo2[p], neg1, hhi2[p]);
+                hlo2[p] = fadd2(lo2[p], cz2[p]);
             }
             cur_j = j;
         }
         const u64 s2 = pack2(s, s);
+        if (full) {
 #pragma unroll
-        for (int p = 0; p < CPT / 2; ++p) {
-            const u64 o = ffma2(s2, hd2[p], hlo2[p]);
-            if (cok[2 * p]) orow[64 * p] = lo_of(o);
-            if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
+            for (int p = 0; p < CPT / 2; ++p) {
+                const u64 o = ffma2(s2, hd2[p], hlo2[p]);
+                orow[64 * p] = lo_of(o);
+                orow[64 * p + 32] = hi_of(o);
+            }
+        } else {
+#pragma unroll
+            for (int p = 0; p < CPT / 2; ++p) {
+                const u64 o = ffma2(s2, hd2[p], hlo2[p]);
+                if (cok[2 * p]) orow[64 * p] = lo_of(o);
+                if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
+            }
         }
     }
 }

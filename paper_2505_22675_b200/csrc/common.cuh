@@ -103,16 +103,16 @@ __device__ __forceinline__ u64 pack2(float lo, float hi)
 }
 __device__ __forceinline__ float lo_of(u64 v)
 {
-    float lo, hi;
+    float lo;
+    float hi __attribute__((unused));
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-    (void)hi;
     return lo;
 }
 __device__ __forceinline__ float hi_of(u64 v)
 {
-    float lo, hi;
+    float lo __attribute__((unused));
+    float hi;
     asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-    (void)lo;
     return hi;
 }
 __device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c)
