@@ -297,7 +297,9 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.workload]["label"], "nodes_per_step_per_gpu": nodes_per_step,
                    "soundings": int(sw.x.shape[0]), "k": sw.k,
-                   "l2": "grid inputs+outputs (%.0f MB per method) exceed the 126 MB L2; no flush" % (grid_bytes / 1e6)
+                   "l2": ("grid inputs+outputs (%.0f MB per method) exceed the 126 MB L2; the kriging soundings (%.0f MB) are "
+                          "evicted every step by the %.0f MB the two grid methods stream through L2 before it; no explicit flush"
+                          % (grid_bytes / 1e6, 16.0 * sw.x.shape[0] / 1e6, 2 * grid_bytes / 1e6))
                    if grid_bytes > 2.0e8 else "grid data fits L2: warm-L2 numbers for bilinear/spline",
                    "parallelism": f"replicated batches x{world}, no collective"},
         "methods": meth,
