@@ -135,6 +135,13 @@ BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram
 /* Releases an index (synchronises the device first).  NULL is a no-op. */
 BATHY_API void krige_free_index(krige_index_t* idx);
 
+/* Stream-ordered release, no host synchronisation: the index memory returns to the device's memory
+ * pool when `cuda_stream` reaches this point.  The caller guarantees that every krige_predict that
+ * uses the index was issued on `cuda_stream` before this call (or is otherwise ordered before it).
+ * The handle is invalid on return.  NULL is a no-op.  (Real-time tile loop: build, predict tiles,
+ * release -- without ever stalling the host.) */
+BATHY_API void krige_free_index_async(krige_index_t* idx, void* cuda_stream);
+
 /* Introspection of an index (host values, valid after build): number of soundings, cell size used,
  * cell-grid dimensions. */
 BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell_size, int32_t* ncx, int32_t* ncy);

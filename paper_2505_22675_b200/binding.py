@@ -22,7 +22,7 @@ EXPONENTIAL, SPHERICAL = 0, 1
 MAX_K = 64
 
 SYMBOLS = ["interp_bilinear", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
-           "krige_predict", "krige_free_index", "krige_index_info", "interp_bilinear_host",
+           "krige_predict", "krige_free_index", "krige_free_index_async", "krige_index_info", "interp_bilinear_host",
            "interp_spline_host", "krige_host", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path"]
 
 
@@ -61,6 +61,8 @@ def lib():
         L.krige_predict.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, vp, vp, vp]
         L.krige_free_index.argtypes = [vp]
         L.krige_free_index.restype = None
+        L.krige_free_index_async.argtypes = [vp, vp]
+        L.krige_free_index_async.restype = None
         L.krige_index_info.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_float),
                                        C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.interp_bilinear_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
@@ -154,6 +156,12 @@ class KrigeIndex:
     def free(self):
         if self.handle:
             lib().krige_free_index(self.handle)
+            self.handle = None
+
+    def free_async(self, stream=None):
+        """Stream-ordered release (krige_free_index_async): no host synchronisation."""
+        if self.handle:
+            lib().krige_free_index_async(self.handle, _stream(stream))
             self.handle = None
 
     def __del__(self):

@@ -10,6 +10,7 @@ size_t spline_workspace_bytes(const grid_geom_t&, const grid_geom_t&);
 int launch_spline(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t, int path);
 int build_index(const float*, const float*, const float*, int64_t, float, cudaStream_t, krige_index**);
 void free_index(krige_index*);
+void free_index_async(krige_index*, cudaStream_t);
 int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, int, float*, int32_t*, int64_t*,
                    cudaStream_t);
 
@@ -94,6 +95,7 @@ BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram
 }
 
 BATHY_API void krige_free_index(krige_index_t* idx) { free_index(idx); }
+BATHY_API void krige_free_index_async(krige_index_t* idx, void* cuda_stream) { free_index_async(idx, static_cast<cudaStream_t>(cuda_stream)); }
 
 BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell_size, int32_t* ncx, int32_t* ncy)
 {

@@ -186,11 +186,29 @@ inline int grid_for(int64_t n)
 
 }  // namespace
 
+
+// The default memory pool gives freed blocks back to the driver at every synchronisation unless its
+// release threshold is raised; with it raised, cudaMallocAsync of the index and its scratch is a
+// pointer bump after the first call.  Once per device.
+static void pool_keep_warm()
+{
+    static bool done[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64 || done[dev]) return;
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        unsigned long long keep = 1ull << 31;              // hold up to 2 GiB of freed blocks
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    done[dev] = true;
+}
+
 int build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n, float cell_size,
                 cudaStream_t stream, krige_index** out_index)
 {
     *out_index = nullptr;
     // 1. bounding box
+    pool_keep_warm();
     const int nb = grid_for(n);
     float4* d_partial = nullptr;
     BATHY_CUDA_TRY(cudaMallocAsync(&d_partial, sizeof(float4) * (size_t)(nb + 1), stream));
@@ -247,8 +265,10 @@ int build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n,
     int32_t* d_cursor = nullptr;
     int32_t* d_sums = nullptr;
     const int nsb = (int)((ncells + kScanBlock - 1) / kScanBlock);
-    cudaError_t e = cudaMalloc(&idx->d_pts, sizeof(float4) * (size_t)n);
-    if (e == cudaSuccess) e = cudaMalloc(&idx->d_cell_start, sizeof(int32_t) * (size_t)(ncells + 1));
+    // stream-ordered allocations from the device's default pool (kept warm, see pool_keep_warm):
+    // a synchronous cudaMalloc costs more than all the kernels of the build together
+    cudaError_t e = cudaMallocAsync(&idx->d_pts, sizeof(float4) * (size_t)n, stream);
+    if (e == cudaSuccess) e = cudaMallocAsync(&idx->d_cell_start, sizeof(int32_t) * (size_t)(ncells + 1), stream);
     if (e == cudaSuccess) e = cudaMallocAsync(&d_tmp, sizeof(float4) * (size_t)n, stream);
     if (e == cudaSuccess) e = cudaMallocAsync(&d_cursor, sizeof(int32_t) * (size_t)(ncells + 1), stream);
     if (e == cudaSuccess) e = cudaMallocAsync(&d_sums, sizeof(int32_t) * (size_t)(nsb + 1), stream);
@@ -258,7 +278,8 @@ int build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n,
         if (d_tmp) cudaFreeAsync(d_tmp, stream);
         if (d_cursor) cudaFreeAsync(d_cursor, stream);
         if (d_sums) cudaFreeAsync(d_sums, stream);
-        cudaFree(idx->d_pts); cudaFree(idx->d_cell_start);
+        if (idx->d_pts) cudaFreeAsync(idx->d_pts, stream);
+        if (idx->d_cell_start) cudaFreeAsync(idx->d_cell_start, stream);
         delete idx;
         return BATHY_ERR_CUDA;
     }
@@ -278,7 +299,8 @@ int build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n,
     cudaFreeAsync(d_cursor, stream);
     cudaFreeAsync(d_sums, stream);
     if (st != BATHY_OK) {
-        cudaFree(idx->d_pts); cudaFree(idx->d_cell_start);
+        if (idx->d_pts) cudaFreeAsync(idx->d_pts, stream);
+        if (idx->d_cell_start) cudaFreeAsync(idx->d_cell_start, stream);
         delete idx;
         return st;
     }
@@ -292,8 +314,19 @@ void free_index(krige_index* idx)
     if (!idx || idx->magic != kIndexMagic) return;
     cudaDeviceSynchronize();
     idx->magic = 0;
-    cudaFree(idx->d_pts);
-    cudaFree(idx->d_cell_start);
+    cudaFreeAsync(idx->d_pts, 0);                          // (the device is idle: synchronised above)
+    cudaFreeAsync(idx->d_cell_start, 0);
+    delete idx;
+}
+
+// Stream-ordered release: the memory goes back to the pool when `stream` reaches this point; no host
+// synchronisation.
+void free_index_async(krige_index* idx, cudaStream_t stream)
+{
+    if (!idx || idx->magic != kIndexMagic) return;
+    idx->magic = 0;
+    cudaFreeAsync(idx->d_pts, stream);
+    cudaFreeAsync(idx->d_cell_start, stream);
     delete idx;
 }
 

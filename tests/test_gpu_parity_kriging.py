@@ -224,3 +224,21 @@ def test_large_coordinates_and_clustered_density():
     outside = (np.abs(xx - 102) > 8) | (np.abs(yy - 102) > 8)
     assert err[outside].max() <= TOL * depth_range(ref["zhat"])
     assert err.max() <= 0.5
+
+
+def test_stream_ordered_release_and_rebuild():
+    """krige_free_index_async: build -> predict -> release -> build again on the same stream, no host
+    synchronisation in between; results are bit-identical from call to call."""
+    b = _bathy()
+    w = W.sounding_config(4, width=120.0, n_target=3600, n_out=64)
+    xt, yt, zt = (torch.from_numpy(a).cuda() for a in (w.x, w.y, w.z))
+    outs = []
+    for _ in range(4):
+        idx = b.krige_build_index(xt, yt, zt)
+        outs.append(b.krige_predict(idx, w.geom_out, w.model, w.range_, w.sill, w.nugget, w.k))
+        idx.free_async()
+        assert idx.handle is None
+    torch.cuda.synchronize()
+    for o in outs[1:]:
+        assert torch.equal(o, outs[0])
+    assert torch.isfinite(outs[0]).all()
