@@ -78,7 +78,8 @@ struct __align__(16) WarpSmem {
     float    nb_x[S::NB][S::XYS];               // neighbour coordinates, scaled, relative to the block centre
     float    nb_y[S::NB][S::XYS];
     float    nb_z[S::NB][K];                    // neighbour depths
-    float2   cxy[S::CAP];                       // candidates: coordinates as given (fp32)
+    float    cx[S::CAP];                        // candidates: coordinates as given (fp32), as two planes so
+    float    cy[S::CAP];                        //             that two candidates load as one fp32x2 pair
     float    cz[S::CAP];                        //             depth (pilot: key bits)
     int32_t  cid[S::CAP];                       //             original index
     uint16_t hist[kBuckets + 1][32];            // per-lane key histogram (column = lane)
@@ -239,11 +240,25 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
 #pragma unroll
     for (int b = 0; b <= kBuckets; ++b) ws.hist[b][lane] = (uint16_t)0;
     // pass 1: histogram of the keys
-#pragma unroll 4
-    for (int c = 0; c < n_c; ++c) {
-        const float2 xy = ws.cxy[c];
-        const float key = knn_key(xq, yq, xy.x, xy.y);
-        if (key <= hi) ws.hist[bucket_of(key, scale)][lane] += (uint16_t)1;
+    // Two candidates at a time in packed fp32x2 arithmetic: every operation is the round-to-nearest
+    // operation of reading K2 (x*(-1) + xq is exactly xq - x), so the keys are bit-identical to knn_key.
+    // (The caller pads an odd list with a candidate at infinity: its key is +inf.)
+    const u64 xq2 = pack2(xq, xq), yq2 = pack2(yq, yq), neg1 = pack2(-1.0f, -1.0f);
+    const u64 sc2 = pack2(scale, scale), mg2 = pack2(12582912.0f, 12582912.0f);
+    auto keys2 = [&](int c, float& k0, float& k1, int& b0, int& b1) {
+        const u64 X = *reinterpret_cast<const u64*>(&ws.cx[c]), Y = *reinterpret_cast<const u64*>(&ws.cy[c]);
+        const u64 dx = ffma2(X, neg1, xq2), dy = ffma2(Y, neg1, yq2);
+        const u64 kk = ffma2(dx, dx, fmul2(dy, dy));
+        const u64 bb = ffma2(kk, sc2, mg2);
+        k0 = lo_of(kk); k1 = hi_of(kk);
+        b0 = __float_as_int(lo_of(bb)) - 0x4B400000; b1 = __float_as_int(hi_of(bb)) - 0x4B400000;
+    };
+#pragma unroll 2
+    for (int c = 0; c < n_c; c += 2) {
+        float k0, k1; int b0, b1;
+        keys2(c, k0, k1, b0, b1);
+        if (k0 <= hi) ws.hist[b0][lane] += (uint16_t)1;
+        if (k1 <= hi) ws.hist[b1][lane] += (uint16_t)1;
     }
     // the bucket that holds the k-th key
     int bstar = kBuckets + 1, below = 0, cum = 0;
@@ -257,27 +272,30 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     if (bstar > kBuckets) return false;
     // pass 2: everything below the critical bucket is a neighbour; the critical bucket is listed
     int cnt = 0, ncrit = 0;
-#pragma unroll 4
-    for (int c = 0; c < n_c; ++c) {
-        const float2 xy = ws.cxy[c];
-        const float key = knn_key(xq, yq, xy.x, xy.y);
-        if (key <= hi) {
-            const int b = bucket_of(key, scale);
-            if (b < bstar) { ws.nbl[cnt][lane] = (uint16_t)c; ++cnt; }
-            else if (b == bstar) { if (ncrit < kCrit) ws.crit[ncrit][lane] = (uint16_t)c; ++ncrit; }
+#pragma unroll 2
+    for (int c = 0; c < n_c; c += 2) {
+        float k0, k1; int b0, b1;
+        keys2(c, k0, k1, b0, b1);
+        if (k0 <= hi) {
+            if (b0 < bstar) { ws.nbl[cnt][lane] = (uint16_t)c; ++cnt; }
+            else if (b0 == bstar) { if (ncrit < kCrit) ws.crit[ncrit][lane] = (uint16_t)c; ++ncrit; }
+        }
+        if (k1 <= hi) {
+            if (b1 < bstar) { ws.nbl[cnt][lane] = (uint16_t)(c + 1); ++cnt; }
+            else if (b1 == bstar) { if (ncrit < kCrit) ws.crit[ncrit][lane] = (uint16_t)(c + 1); ++ncrit; }
         }
     }
     const int need = k - below;                            // >= 1 candidates of the critical bucket
     if (ncrit <= kCrit) {
         for (int e = 0; e < ncrit; ++e) {                  // rank by (key, index) inside the bucket
             const int ce = ws.crit[e][lane];
-            const float2 xe = ws.cxy[ce];
+            const float2 xe = make_float2(ws.cx[ce], ws.cy[ce]);
             const uint32_t ke = __float_as_uint(knn_key(xq, yq, xe.x, xe.y));
             const int32_t ie = ws.cid[ce];
             int rank = 0;
             for (int f = 0; f < ncrit; ++f) {
                 const int cf = ws.crit[f][lane];
-                const float2 xf = ws.cxy[cf];
+                const float2 xf = make_float2(ws.cx[cf], ws.cy[cf]);
                 const uint32_t kf = __float_as_uint(knn_key(xq, yq, xf.x, xf.y));
                 const int32_t jf = ws.cid[cf];
                 rank += (kf < ke || (kf == ke && jf < ie)) ? 1 : 0;
@@ -290,7 +308,7 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
         for (int t = 0; t < need; ++t) {
             uint32_t bk = 0xffffffffu; int32_t bi = 0x7fffffff; int bc = -1;
             for (int c = 0; c < n_c; ++c) {
-                const float2 xy = ws.cxy[c];
+                const float2 xy = make_float2(ws.cx[c], ws.cy[c]);
                 const float key = knn_key(xq, yq, xy.x, xy.y);
                 if (!(key <= hi) || bucket_of(key, scale) != bstar) continue;
                 const uint32_t kc = __float_as_uint(key);
@@ -315,13 +333,13 @@ __device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSme
     const int k = p.k;
     for (int e = 0; e < k; ++e) {
         const int ce = ws.nbl[e][lane];
-        const float2 xe = ws.cxy[ce];
+        const float2 xe = make_float2(ws.cx[ce], ws.cy[ce]);
         const uint32_t ke = __float_as_uint(knn_key(xq, yq, xe.x, xe.y));
         const int32_t ie = ws.cid[ce];
         int rank = 0;
         for (int f = 0; f < k; ++f) {
             const int cf = ws.nbl[f][lane];
-            const float2 xf = ws.cxy[cf];
+            const float2 xf = make_float2(ws.cx[cf], ws.cy[cf]);
             const uint32_t kf = __float_as_uint(knn_key(xq, yq, xf.x, xf.y));
             const int32_t jf = ws.cid[cf];
             rank += (kf < ke || (kf == ke && jf < ie)) ? 1 : 0;
@@ -533,7 +551,8 @@ krige_predict_kernel(const PredictParams p)
                                      return fmaf(ax, ax, ay * ay) <= Rb2;
                                  },
                                  [&](int slot, const float4& pt) {
-                                     ws.cxy[slot] = make_float2(pt.x, pt.y);
+                                     ws.cx[slot] = pt.x;
+                                     ws.cy[slot] = pt.y;
                                      ws.cz[slot] = pt.z;
                                      ws.cid[slot] = __float_as_int(pt.w);
                                  });
@@ -541,7 +560,11 @@ krige_predict_kernel(const PredictParams p)
                 if (n_c > S::CAP) {
                     if (sz > 1) { nsub *= 2; s *= 2; continue; }           // split the group and search again
                     group_ok = false;                                      // a single node: degenerate input
+                } else if ((n_c & 1) && lane == 0) {
+                    ws.cx[n_c] = INFINITY;                                 // pad to a whole pair: key = +inf
+                    ws.cy[n_c] = INFINITY;
                 }
+                __syncwarp();
             } else {
                 rho = p.r0;
             }
@@ -579,7 +602,7 @@ krige_predict_kernel(const PredictParams p)
                         const int c = ws.nbl[m < k ? m : 0][sl];
                         z = ws.cz[c];
                         if (m < k) {
-                            const float2 o = ws.cxy[c];
+                            const float2 o = make_float2(ws.cx[c], ws.cy[c]);
                             xy = make_float2(__fmul_rn(o.x - cx, sc), __fmul_rn(o.y - cy, sc));
                         }
                     }
