@@ -17,13 +17,14 @@
 //                instruction, instead of a warp-wide bisection per node.
 //       A candidate list that does not fit splits the block into half blocks (down to single nodes).
 //   K3-K5 solve: G lanes per node (32/G nodes per warp at once), rows of C dealt cyclically to the
-//       lanes and held in REGISTERS (fully unrolled right-looking Cholesky); column j of L is
-//       published through a double-buffered shared-memory column and read back as broadcast float4.
+//       lanes and held in REGISTERS as fp32x2 pairs (fully unrolled right-looking Cholesky, FFMA2
+//       trailing update); column j of L is published through a double-buffered shared-memory column
+//       and read back as broadcast LDS.128.
 //       The three right-hand sides c0, 1 and z ride along as forward substitutions, and
 //           z_hat = y_z.y_c - mu * (y_z.y_1),   mu = (y_1.y_c - 1) / (y_1.y_1),   y_b = L^-1 b
 //       gives the Lagrange/Schur step without any back substitution or explicit weights.
 //       Covariances are built from coordinates relative to the block centre, pre-scaled by
-//       log2(e)/a (exponential) or 1/a (spherical): 7 / 10 instructions a pair.
+//       log2(e)/a (exponential) or 1/a (spherical), two pairs per packed fp32x2 operation.
 //   Tensor cores are not used: the factorisation is a k x k problem with a serial pivot chain.
 #include "krige_index.cuh"
 
@@ -106,23 +107,6 @@ __device__ __forceinline__ float ex2_approx(float v)
     float r;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
     return r;
-}
-
-// Covariance normalised to sill = 1 from the squared distance in SCALED coordinates (h2 > 0):
-// exponential C = cpn exp(-h/a) = 2^(log2 cpn - h log2(e)/a) (PAPER.md:L157, no factor 3);
-// spherical   C = cpn (1 - 1.5 q + 0.5 q^3), q = min(h/a, 1).  h2 == 0 gives NaN (0 * inf): two
-// soundings at one place make the system singular and the node fails (reading K-dup).
-template <int MODEL>
-__device__ __forceinline__ float cov_scaled(float h2, const PredictParams& p)
-{
-    const float rs = rsqrt_approx(h2);
-    if (MODEL == BATHY_VGM_EXPONENTIAL) {
-        return ex2_approx(fmaf(-h2, rs, p.lc));
-    } else {
-        float q;
-        asm("min.NaN.f32 %0, %1, %2;" : "=f"(q) : "f"(h2 * rs), "f"(1.0f));   // NaN (h2 == 0) survives
-        return fmaf(q, fmaf(q * q, p.c05, p.c15), p.cpn);
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -348,8 +332,12 @@ __device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSme
     }
 }
 
-// Two covariances at once (see cov_scaled): the distance and polynomial arithmetic is packed, the
-// two rsqrt and the two ex2 go to the MUFU pipe one by one.
+// Two covariances at once, normalised to sill = 1, from squared distances in SCALED coordinates (h2 > 0):
+// exponential C = cpn exp(-h/a) = 2^(log2 cpn - h log2(e)/a) (PAPER.md:L157, no factor 3);
+// spherical   C = cpn (1 - 1.5 q + 0.5 q^3), q = min(h/a, 1).  h2 == 0 gives NaN (0 * inf): two
+// soundings at one place make the system singular and the node fails (reading K-dup).
+// The distance and polynomial arithmetic is packed fp32x2; the two rsqrt and the two ex2 go to the
+// MUFU pipe one by one.
 template <int MODEL>
 __device__ __forceinline__ u64 cov2_scaled(u64 h2, const PredictParams& p)
 {
