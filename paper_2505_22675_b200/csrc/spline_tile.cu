@@ -79,33 +79,25 @@ __device__ __forceinline__ void thomas_window(Rd rd, St st, int k0_rt, int nk_rt
 {
     static_assert(N >= 6, "window too short");
     const int k0 = STATIC ? K0 : k0_rt, nk = STATIC ? NK : nk_rt;
+    // Four passes so that the two serial sweeps are pure register chains (one dependent FMA per knot)
+    // and every shared-memory access sits in a pass without dependencies, all loads in flight at once.
     float e[N];
-    {
-        const float v0 = rd(0);
-        e[1] = fmaf(-1.0f / 6.0f, v0, rd(1));
-    }
 #pragma unroll
-    for (int q = 2; q <= N - 3; ++q) e[q] = fmaf(-cp141(q - 2), e[q - 1], rd(q));
-    {
-        const float vl = rd(N - 1);
-        e[N - 2] = fmaf(-cp141(N - 4), e[N - 3], fmaf(-1.0f / 6.0f, vl, rd(N - 2)));
-    }
+    for (int q = 0; q < N; ++q) e[q] = rd(q);                          // pass 1: the knots
+    e[1] = fmaf(-1.0f / 6.0f, e[0], e[1]);                             // pass 2: forward sweep, e_q in place
+#pragma unroll
+    for (int q = 2; q <= N - 3; ++q) e[q] = fmaf(-cp141(q - 2), e[q - 1], e[q]);
+    e[N - 2] = fmaf(-cp141(N - 4), e[N - 3], fmaf(-1.0f / 6.0f, e[N - 1], e[N - 2]));
+#pragma unroll
+    for (int q = N - 3; q >= 1; --q) e[q] = fmaf(-cp141(q), e[q + 1], e[q]);   // pass 3: backward sweep, wt_q in place
+    // pass 4: M'_q = z_q - 6 c'_q wt_q on the kept knots (the knot is read again: no second register array)
     if (N - 1 - k0 >= 0 && N - 1 - k0 < nk) st(N - 1 - k0, rd(N - 1), 0.0f);
-    float wt = e[N - 2];
-    {
-        const int k = N - 2 - k0;
-        if (k >= 0 && k < nk) {
-            const float v = rd(N - 2);
-            st(k, v, fmaf(-6.0f * cp141(N - 3), wt, v));
-        }
-    }
 #pragma unroll
-    for (int q = N - 3; q >= 1; --q) {
-        wt = fmaf(-cp141(q), wt, e[q]);
+    for (int q = N - 2; q >= 1; --q) {
         const int k = q - k0;
         if (k >= 0 && k < nk) {
             const float v = rd(q);
-            st(k, v, fmaf(-6.0f * cp141(q - 1), wt, v));
+            st(k, v, fmaf(-6.0f * cp141(q - 1), e[q], v));
         }
     }
     if (k0 == 0) st(0, rd(0), 0.0f);
