@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(kTileThreads, 4)
 spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay,
                    const float4* __restrict__ coltab, const float4* __restrict__ rowtab,
                    const int* __restrict__ tbx, const int* __restrict__ tby, const int* __restrict__ rfirst,
-                   int nbx, int n_tiles)
+                   int nbx, int n_tiles, int pf_dist)
 {
     constexpr int TXI = S::TXI, TYI = S::TYI, H = S::H, WX = S::WX, WY = S::WY;
     constexpr int NXI = S::NXI, NYI = S::NYI, PZ = S::PZ, PA = S::PA, PQ = S::PQ;
@@ -196,6 +196,21 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const int nkx = min(NXI, ax.n_in - i0), nky = min(NYI, ay.n_in - j0);   // knots present (last tile may be short)
         issue_load(tile, 0);
         asm volatile("cp.async.commit_group;" ::: "memory");
+        {
+            // L2 prefetch of the window of the tile that starts one wave of CTAs later: its cp.async
+            // then finds the rows in L2 instead of waiting for HBM at the head of the CTA
+            const int pt = tile + pf_dist;
+            if (pt < n_tiles) {
+                const int pbx = pt % nbx, pby = pt / nbx;
+                const int px = min(max(pbx * TXI - H, 0), ax.n_in - WX) & ~31;          // 128-byte lines
+                const int py = min(max(pby * TYI - H, 0), ay.n_in - WY);
+                constexpr int LPR = (WX + 31 + 31) / 32;                               // lines per window row
+                for (int v = tid; v < WY * LPR; v += kTileThreads) {
+                    const int r = v / LPR, c = px + (v - r * LPR) * 32;
+                    if (c < ax.n_in) asm volatile("prefetch.global.L2 [%0];" :: "l"(in + (size_t)(py + r) * ax.n_in + c));
+                }
+            }
+        }
         const int Jbeg = __ldg(tbx + bxt), Jend = __ldg(tbx + bxt + 1);   // output nodes of the tile
         const int Ibeg = __ldg(tby + byt), Iend = __ldg(tby + byt + 1);
         const int offx = w0x & 3;
@@ -384,7 +399,7 @@ int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMa
     if (n_tiles > 0x7fffffffLL) return 1;
     const unsigned ctas = (unsigned)n_tiles;
     spline_tile_kernel<S><<<ctas, kTileThreads, S::smem_bytes, stream>>>(d_in, d_out, ax, ay, coltab, rowtab, tbx, tby, rfirst,
-                                                                          (int)grid.x, (int)n_tiles);
+                                                                          (int)grid.x, (int)n_tiles, 4 * kSMs /* CTAs resident at once */);
     count_launch(2);
     return launch_status();
 }
