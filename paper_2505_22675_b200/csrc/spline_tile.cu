@@ -281,6 +281,14 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 if (__float_as_int(__ldg(rowtab + I).x) < 0)
                     for (int J = Jbeg + lane; J < Jend; J += 32) out[(size_t)I * ax.n_out + J] = qnan;
         }
+        // the row entries (j, s, Cy, Dy) of this warp's band go to shared memory once (the planes of the
+        // sweeps are dead): a global load per row would expose an L2 round trip in every interval
+        constexpr int RT_CAP = (2 * NYI * PZ) / (4 * NW);                 // float4 entries per warp
+        float4* s_rt = reinterpret_cast<float4*>(s_zf) + warp * RT_CAP;
+        const int rt0 = rsv[0], rt_n = rsv[TI] - rsv[0];
+        const bool rt_ok = rt_n <= RT_CAP;                               // warp-uniform
+        if (rt_ok) for (int i = lane; i < rt_n; i += 32) s_rt[i] = __ldg(rowtab + rt0 + i);
+        __syncwarp();
         for (int Jp = Jbeg; Jp < Jend; Jp += 128) {
             const int Jt = Jp + lane;                  // column of e = 0; e-th column is 32 e further
             if (Jt >= Jend) continue;
@@ -343,7 +351,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 if (full) {                            // all four columns inside the tile, no row outside the extent
 #pragma unroll 2
                     for (int r = rs; r < re; ++r, op += ax.n_out) {
-                        const float4 rw = __ldg(rowtab + r);           // (j, s, Cy, Dy)
+                        const float4 rw = rt_ok ? s_rt[r - rt0] : __ldg(rowtab + r);   // (j, s, Cy, Dy)
                         const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
 #pragma unroll
                         for (int p = 0; p < 2; ++p) {
@@ -358,7 +366,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 } else {
 #pragma unroll 1
                     for (int r = rs; r < re; ++r, op += ax.n_out) {
-                        const float4 rw = __ldg(rowtab + r);           // (j, s, Cy, Dy); j < 0: row outside the extent
+                        const float4 rw = rt_ok ? s_rt[r - rt0] : __ldg(rowtab + r);   // (j, s, Cy, Dy); j < 0: outside the extent
                         const bool rv = __float_as_int(rw.x) >= 0;
                         const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
 #pragma unroll
