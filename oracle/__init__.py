@@ -50,6 +50,7 @@ def lib():
         L.oracle_set_num_threads.argtypes = [C.c_int]
         L.oracle_bilinear.argtypes = [fp, gp, gp, dp]
         L.oracle_spline.argtypes = [fp, gp, gp, dp]
+        L.oracle_catmull_rom.argtypes = [fp, gp, gp, dp]
         L.oracle_spline1d.argtypes = [dp, C.c_int, C.c_double, dp, C.c_int, dp, dp]
         L.oracle_node_coords.argtypes = [gp, fp, fp]
         L.oracle_node_coords.restype = None
@@ -108,6 +109,18 @@ def bilinear(z, gi: Geom, go: Geom) -> np.ndarray:
     rc = lib().oracle_bilinear(_p(z, C.c_float), C.byref(gi), C.byref(go), _p(out, C.c_double))
     if rc:
         raise ValueError(f"oracle_bilinear: {rc}")
+    return out
+
+
+def catmull_rom(z, gi: Geom, go: Geom) -> np.ndarray:
+    """4x4 Catmull-Rom cubic, x on 4 rows then y; bilinear fallback when one of the 16
+    neighbours is outside the grid or NaN."""
+    z = _f32(z)
+    assert z.shape == (gi.ny, gi.nx)
+    out = np.empty((go.ny, go.nx), dtype=np.float64)
+    rc = lib().oracle_catmull_rom(_p(z, C.c_float), C.byref(gi), C.byref(go), _p(out, C.c_double))
+    if rc:
+        raise ValueError(f"oracle_catmull_rom: {rc}")
     return out
 
 

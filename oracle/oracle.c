@@ -13,7 +13,8 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): planes, 2.375, knots, S(0.5)=0.6875, S(1.5)=2.2,
  * 0.47265625, M=(0,18/7,-30/7,18/7,0), scipy CubicSpline(natural), two-point closed form
  * lambda1=0.748755187238, equilateral 1/3, constants, sum(lambda)=1, exactness at data, brute-force
- * kNN vs bucket kNN, LU vs numpy.linalg.solve.  No function here is "parity unpinned" against
+ * kNN vs bucket kNN, LU vs numpy.linalg.solve; Catmull-Rom: C(0)=P1, C(1)=P2, C(1/2)=(-P0+9P1+9P2-P3)/16,
+ * quadratics reproduced, NaN/edge fallback = bilinear.  No function here is "parity unpinned" against
  * mathematics; nothing is pinned against the paper's own tables (they need GEBCO).
  */
 #include <math.h>
@@ -98,6 +99,59 @@ int oracle_bilinear(const float *in, const ora_geom *gi, const ora_geom *go, dou
                 double Q22 = in[(size_t)(j + 1) * gi->nx + i + 1];
                 f = (1.0 - t) * (1.0 - s) * Q11 + t * (1.0 - s) * Q21
                   + (1.0 - t) * s * Q12 + t * s * Q22;
+            }
+            out[(size_t)I * go->nx + J] = f;
+        }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ Catmull-Rom cubic
+ * (the paper's own "cubic spline", readings CR1-CR3).
+ * C(t) = 1/2 (2 P1 + (-P0 + P2) t + (2 P0 - 5 P1 + 4 P2 - P3) t^2 + (-P0 + 3 P1 - 3 P2 + P3) t^3)
+ * (eq. at), P0..P3 the samples at i-1, i, i+1, i+2, t = u - i. */
+static double catmull_rom(double P0, double P1, double P2, double P3, double t)
+{
+    return 0.5 * (2.0 * P1 + (-P0 + P2) * t + (2.0 * P0 - 5.0 * P1 + 4.0 * P2 - P3) * t * t
+                  + (-P0 + 3.0 * P1 - 3.0 * P2 + P3) * t * t * t);
+}
+
+/* "first interpolates in x on each of 4 rows, and then in y".  Interval location as
+ * bilinear (B1, B2, B4).  CR2/CR3: if any of the 16 neighbours lies outside the grid or is NaN the node
+ * "falls back to a bilinear calculation" (sense fixed by L171), i.e. the value of
+ * oracle_bilinear at that node (NaN if one of its 4 corners is NaN: bilinear has no fallback, L182). */
+int oracle_catmull_rom(const float *in, const ora_geom *gi, const ora_geom *go, double *out)
+{
+    if (!in || !out || gi->nx < 2 || gi->ny < 2 || go->nx < 1 || go->ny < 1) return -1;
+    if (!(gi->dx > 0.0f) || !(gi->dy > 0.0f)) return -1;
+    #pragma omp parallel for schedule(static)
+    for (int I = 0; I < go->ny; ++I) {
+        double s;
+        int j = locate(node_v(gi, go, I), gi->ny, &s);
+        for (int J = 0; J < go->nx; ++J) {
+            double t;
+            int i = locate(node_u(gi, go, J), gi->nx, &t);
+            double f = NAN;
+            if (i >= 0 && j >= 0) {
+                int all16 = (i - 1 >= 0) && (i + 2 <= gi->nx - 1) && (j - 1 >= 0) && (j + 2 <= gi->ny - 1);
+                double R[4];
+                if (all16) {
+                    for (int b = 0; b < 4 && all16; ++b) {
+                        const float *row = in + (size_t)(j - 1 + b) * gi->nx + (i - 1);
+                        for (int a = 0; a < 4; ++a) if (isnan(row[a])) all16 = 0;
+                        R[b] = catmull_rom(row[0], row[1], row[2], row[3], t);
+                    }
+                }
+                if (all16) {
+                    f = catmull_rom(R[0], R[1], R[2], R[3], s);
+                } else {
+                    double Q11 = in[(size_t)j * gi->nx + i];
+                    double Q21 = in[(size_t)j * gi->nx + i + 1];
+                    double Q12 = in[(size_t)(j + 1) * gi->nx + i];
+                    double Q22 = in[(size_t)(j + 1) * gi->nx + i + 1];
+                    f = (1.0 - t) * (1.0 - s) * Q11 + t * (1.0 - s) * Q21
+                      + (1.0 - t) * s * Q12 + t * s * Q22;
+                }
             }
             out[(size_t)I * go->nx + J] = f;
         }
