@@ -84,6 +84,17 @@ typedef struct krige_index krige_index_t;
 BATHY_API int interp_bilinear(const float* d_in, grid_geom_t in, float* d_out, grid_geom_t out, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * interp_catmull_rom -- the paper's own "cubic spline" (section III-B; SURVEY.md
+ * 8(f) NEXT-1).  Interval location, extent and layout as interp_bilinear.  With P0..P3 the samples at
+ * i-1, i, i+1, i+2 and t = u - i,
+ *   C(t) = 1/2 (2 P1 + (-P0 + P2) t + (2 P0 - 5 P1 + 4 P2 - P3) t^2 + (-P0 + 3 P1 - 3 P2 + P3) t^3)
+ * is applied in x on each of the 4 rows j-1 .. j+2 and then in y (L138).  A node with
+ * one of its 16 neighbours outside the grid or NaN "falls back to a bilinear calculation" (L144, sense
+ * fixed by L171): it gets the value of interp_bilinear (NaN if one of the 4 corners is NaN, L182).
+ * d_in  [in.ny * in.nx] fp32, read only.   d_out [out.ny * out.nx] fp32, fully overwritten; no overlap. */
+BATHY_API int interp_catmull_rom(const float* d_in, grid_geom_t in, float* d_out, grid_geom_t out, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * interp_spline -- separable natural bicubic spline (BASELINE.json north_star; DESIGN.md reading
  * D1: the paper's section III-B, uses the local Catmull-Rom cubic instead).
  * 1-D operator on uniform knots with spacing h: second derivatives M with M_0 = M_{n-1} = 0 and

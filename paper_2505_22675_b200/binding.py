@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libbathy.so")
 EXPONENTIAL, SPHERICAL = 0, 1
 MAX_K = 64
 
-SYMBOLS = ["interp_bilinear", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
+SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
            "krige_predict", "krige_free_index", "krige_free_index_async", "krige_index_info", "interp_bilinear_host",
            "interp_spline_host", "krige_host", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path"]
 
@@ -54,6 +54,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         vp = C.c_void_p
         L.interp_bilinear.argtypes = [vp, GridGeom, vp, GridGeom, vp]
+        L.interp_catmull_rom.argtypes = [vp, GridGeom, vp, GridGeom, vp]
         L.interp_spline_workspace_bytes.argtypes = [GridGeom, GridGeom]
         L.interp_spline_workspace_bytes.restype = C.c_size_t
         L.interp_spline.argtypes = [vp, GridGeom, vp, GridGeom, vp, C.c_size_t, vp]
@@ -118,6 +119,20 @@ def interp_bilinear(z: torch.Tensor, gin, gout, out: torch.Tensor | None = None,
     _dev_f32(out, "out")
     assert out.numel() == go.nx * go.ny
     _check(lib().interp_bilinear(z.data_ptr(), gi, out.data_ptr(), go, _stream(stream)), "interp_bilinear")
+    return out
+
+
+def interp_catmull_rom(z: torch.Tensor, gin, gout, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """PAPER.md:L136-L144 (the paper's own cubic): 4x4 Catmull-Rom, bilinear fallback where one of the 16
+    neighbours is missing.  z [ny_in, nx_in] fp32 on the GPU -> [ny_out, nx_out]."""
+    gi, go = _geom(gin), _geom(gout)
+    _dev_f32(z, "z")
+    assert z.numel() == gi.nx * gi.ny
+    if out is None:
+        out = torch.empty((go.ny, go.nx), dtype=torch.float32, device=z.device)
+    _dev_f32(out, "out")
+    assert out.numel() == go.nx * go.ny
+    _check(lib().interp_catmull_rom(z.data_ptr(), gi, out.data_ptr(), go, _stream(stream)), "interp_catmull_rom")
     return out
 
 

@@ -6,6 +6,7 @@
 namespace bathy {
 
 int launch_bilinear(const float*, const grid_geom_t&, float*, const grid_geom_t&, cudaStream_t);
+int launch_catmull_rom(const float*, const grid_geom_t&, float*, const grid_geom_t&, cudaStream_t);
 size_t spline_workspace_bytes(const grid_geom_t&, const grid_geom_t&);
 int launch_spline(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t, int path);
 int build_index(const float*, const float*, const float*, int64_t, float, cudaStream_t, krige_index**);
@@ -49,6 +50,16 @@ BATHY_API int interp_bilinear(const float* d_in, grid_geom_t in, float* d_out, g
     rc = check_out_geom(out);
     if (rc) return rc;
     return launch_bilinear(d_in, in, d_out, out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+BATHY_API int interp_catmull_rom(const float* d_in, grid_geom_t in, float* d_out, grid_geom_t out, void* cuda_stream)
+{
+    if (!d_in || !d_out) return BATHY_ERR_NULL;
+    int rc = check_in_geom(in);
+    if (rc) return rc;
+    rc = check_out_geom(out);
+    if (rc) return rc;
+    return launch_catmull_rom(d_in, in, d_out, out, static_cast<cudaStream_t>(cuda_stream));
 }
 
 BATHY_API size_t interp_spline_workspace_bytes(grid_geom_t in, grid_geom_t out)

@@ -1,0 +1,234 @@
+// catmull_rom.cu -- interp_catmull_rom: the paper's own "cubic spline" (formula at
+// L140).  4 x 4 neighbours, x on each of the 4 rows, then y; a node with one of
+// its 16 neighbours outside the grid or NaN falls back to bilinear (sense fixed by L171;
+// DESIGN.md readings CR1-CR3).
+//
+// Same skeleton as bilinear.cu: one CTA owns a TW x TH output tile, stages the covering input
+// footprint (+2 samples of halo) in shared memory by cp.async, a thread owns CPT lane-contiguous
+// columns and marches down the rows.  Per column it keeps, for the 4 input rows j-1 .. j+2 around the
+// current row interval, the x-direction cubic X and the x-direction linear interpolant L (for the
+// fallback), all on (sample - z_ref).  When the output row enters the next interval the window of
+// rows shifts by one and ONE new row is evaluated (4 shared loads, 6 FMA); a node then costs the
+// 4-term y cubic, the 1-term y lerp and a select.
+// The printed polynomial is evaluated as weights w_k(t) (they sum to 1, so subtracting z_ref is exact
+// algebra):  w0 = (-t + 2t^2 - t^3)/2, w1 = (2 - 5t^2 + 3t^3)/2, w2 = (t + 4t^2 - 3t^3)/2,
+// w3 = (-t^2 + t^3)/2.
+#include "common.cuh"
+
+namespace bathy {
+
+namespace {
+
+constexpr int kThreads = 256;
+
+__device__ __forceinline__ float4 cr_weights(float t)
+{
+    const float t2 = t * t, t3 = t2 * t;
+    return make_float4(0.5f * (-t + 2.0f * t2 - t3), 0.5f * (2.0f - 5.0f * t2 + 3.0f * t3),
+                       0.5f * (t + 4.0f * t2 - 3.0f * t3), 0.5f * (-t2 + t3));
+}
+
+template <int CPT, int TH>
+__global__ void __launch_bounds__(kThreads)
+catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay)
+{
+    constexpr int TW = CPT * kThreads;
+    extern __shared__ __align__(16) float s_tile[];   // [fh][pitch] raw input samples of the tile's footprint
+    __shared__ float4 s_wy[TH];                       // y weights of the output row
+    __shared__ int2   s_row[TH];                      // (input row j or -1, float bits of s) per output row
+    __shared__ int    s_bounds[4];                    // i_lo, i_hi, j_lo, j_hi (interval bounds of the tile)
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int J0 = blockIdx.x * TW;
+    const int I0 = blockIdx.y * TH;
+    const int Jlast = min(J0 + TW, ax.n_out) - 1;
+    const int Ilast = min(I0 + TH, ay.n_out) - 1;
+    const int nrows = Ilast - I0 + 1;
+
+    if (tid == 0) s_bounds[0] = axis_clamped(ax, J0);
+    if (tid == 1) s_bounds[1] = axis_clamped(ax, Jlast) + 1;
+    if (tid == 2) s_bounds[2] = axis_clamped(ay, I0);
+    if (tid == 3) s_bounds[3] = axis_clamped(ay, Ilast) + 1;
+    if (tid >= 32 && tid < 32 + TH) {
+        float s = 0.0f;
+        const int r = tid - 32;
+        const int j = (r < nrows) ? axis_locate(ay, I0 + r, &s) : -1;
+        s_row[r] = make_int2(j, __float_as_int(j < 0 ? 0.0f : s));
+        s_wy[r] = cr_weights(j < 0 ? 0.0f : s);
+    }
+    __syncthreads();
+    // footprint: the intervals' samples plus one more sample on every side, clipped to the grid
+    const int fi0 = max(s_bounds[0] - 1, 0), fi1 = min(s_bounds[1] + 1, ax.n_in - 1);
+    const int fj0 = max(s_bounds[2] - 1, 0), fj1 = min(s_bounds[3] + 1, ay.n_in - 1);
+    const int fw = fi1 - fi0 + 1, fh = fj1 - fj0 + 1;
+
+    const int a_lo = fi0 & ~3, offx = fi0 - a_lo;
+    const int pitch = (fw + 6) & ~3;                  // >= offx + fw, a multiple of 4
+    if ((reinterpret_cast<uintptr_t>(in) & 15) == 0 && (ax.n_in & 3) == 0) {
+        const int vpr = pitch >> 2;
+        for (int v = tid; v < fh * vpr; v += kThreads) {
+            const int r = v / vpr, c4 = (v - r * vpr) << 2;
+            const int col = a_lo + c4;
+            const int bytes = max(0, min(16, (ax.n_in - col) * 4));      // past the row end: zero fill
+            const float* src = in + (size_t)(fj0 + r) * ax.n_in + min(col, ax.n_in - 4);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + c4);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(bytes) : "memory");
+        }
+    } else {
+        for (int v = tid; v < fh * fw; v += kThreads) {
+            const int r = v / fw, c = v - r * fw;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + offx + c);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(dst), "l"(in + (size_t)(fj0 + r) * ax.n_in + fi0 + c) : "memory");
+        }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    float zref = __ldg(in + (size_t)fj0 * ax.n_in + fi0);
+    if (!isfinite(zref)) zref = 0.0f;
+
+    // this thread's columns
+    const int Jt = J0 + warp * (32 * CPT) + lane;     // column of e = 0
+    bool cok[CPT], c4ok[CPT];                         // column inside the tile / has its 4 x neighbours in the grid
+    float ct[CPT], cnan[CPT];
+    float4 cw[CPT];
+    int c0[CPT], c1[CPT], c2[CPT], c3[CPT];           // offsets of P0..P3 in a footprint row (clamped into it)
+    const float qnan = __int_as_float(0x7fc00000);
+#pragma unroll
+    for (int e = 0; e < CPT; ++e) {
+        const int J = Jt + 32 * e;
+        cok[e] = J <= Jlast;
+        ct[e] = 0.0f;
+        const int i = cok[e] ? axis_locate(ax, J, &ct[e]) : -1;
+        cnan[e] = (i < 0) ? qnan : 0.0f;
+        const int ic = (i < 0) ? fi0 : i;             // a column outside the extent still reads inside the footprint
+        c4ok[e] = (i >= 1) && (i + 2 <= ax.n_in - 1);
+        cw[e] = cr_weights(ct[e]);
+        c1[e] = min(max(ic, fi0), fi1 - 1) - fi0 + offx;
+        c2[e] = c1[e] + 1;
+        c0[e] = max(c1[e] - 1, offx);
+        c3[e] = min(c1[e] + 2, fi1 - fi0 + offx);
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+
+    // x cubic X and x lerp L of footprint row fr at this thread's columns (on sample - z_ref)
+    auto row_eval = [&](int jrow, float* X, float* L) {
+        const bool in_grid = jrow >= 0 && jrow <= ay.n_in - 1;
+        const float* row = s_tile + (min(max(jrow, fj0), fj1) - fj0) * pitch;
+#pragma unroll
+        for (int e = 0; e < CPT; ++e) {
+            const float p0 = row[c0[e]] - zref, p1 = row[c1[e]] - zref, p2 = row[c2[e]] - zref, p3 = row[c3[e]] - zref;
+            const float x = fmaf(cw[e].w, p3, fmaf(cw[e].z, p2, fmaf(cw[e].y, p1, cw[e].x * p0)));
+            X[e] = (in_grid && c4ok[e]) ? x : qnan;   // NaN marks "one of the row's 4 neighbours is missing"
+            L[e] = fmaf(ct[e], p2 - p1, p1);
+        }
+    };
+
+    float X[4][CPT], L[4][CPT];                       // rows j-1 .. j+2
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+        for (int e = 0; e < CPT; ++e) X[b][e] = L[b][e] = 0.0f;
+    int cur_j = -5;
+    float* orow = out + (size_t)I0 * ax.n_out + Jt;
+    for (int r = 0; r < nrows; ++r, orow += ax.n_out) {
+        const int2 rw = s_row[r];
+        const int j = rw.x;
+        if (j < 0) {                                   // CTA-uniform: row outside the input extent
+#pragma unroll
+            for (int e = 0; e < CPT; ++e) if (cok[e]) orow[32 * e] = qnan;
+            continue;
+        }
+        if (j != cur_j) {                              // CTA-uniform: the window of 4 input rows moves
+            if (j == cur_j + 1) {
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+#pragma unroll
+                    for (int e = 0; e < CPT; ++e) { X[b][e] = X[b + 1][e]; L[b][e] = L[b + 1][e]; }
+                row_eval(j + 2, X[3], L[3]);
+            } else {
+#pragma unroll
+                for (int b = 0; b < 4; ++b) row_eval(j - 1 + b, X[b], L[b]);
+            }
+            cur_j = j;
+        }
+        const float s = __int_as_float(rw.y);
+        const float4 wy = s_wy[r];
+#pragma unroll
+        for (int e = 0; e < CPT; ++e) {
+            const float cub = fmaf(wy.w, X[3][e], fmaf(wy.z, X[2][e], fmaf(wy.y, X[1][e], wy.x * X[0][e])));
+            const float bil = fmaf(s, L[2][e] - L[1][e], L[1][e]);
+            // cub is NaN exactly when one of the 16 neighbours is outside the grid or NaN (0 * NaN = NaN)
+            const float v = ((cub == cub) ? cub : bil) + zref + cnan[e];
+            if (cok[e]) orow[32 * e] = v;
+        }
+    }
+}
+
+// Any geometry (including strong down-sampling, where a tile's input footprint does not fit in
+// shared memory): one thread per output node, the 16 neighbours through the read-only path.
+__global__ void __launch_bounds__(kThreads)
+catmull_rom_gather_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay)
+{
+    const int J = blockIdx.x * kThreads + threadIdx.x;
+    if (J >= ax.n_out) return;
+    float t, s;
+    const int i = axis_locate(ax, J, &t);
+    const float4 wx = cr_weights(t);
+    const bool c4ok = (i >= 1) && (i + 2 <= ax.n_in - 1);
+    for (int I = blockIdx.y; I < ay.n_out; I += gridDim.y) {
+        const int j = axis_locate(ay, I, &s);
+        float f = __int_as_float(0x7fc00000);
+        if (i >= 0 && j >= 0) {
+            const float* p = in + (size_t)j * ax.n_in + i;
+            const float zref = __ldg(p);
+            const float q11 = __ldg(p) - zref, q21 = __ldg(p + 1) - zref;
+            const float q12 = __ldg(p + ax.n_in) - zref, q22 = __ldg(p + ax.n_in + 1) - zref;
+            const float lo = fmaf(t, q21 - q11, q11), hi = fmaf(t, q22 - q12, q12);
+            f = fmaf(s, hi - lo, lo);                              // the bilinear fallback (NaN if a corner is NaN)
+            const bool zok = zref == zref;
+            if (zok && c4ok && j >= 1 && j + 2 <= ay.n_in - 1) {
+                const float4 wy = cr_weights(s);
+                const float wyv[4] = {wy.x, wy.y, wy.z, wy.w};
+                float cub = 0.0f;
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const float* r = p + (ptrdiff_t)(b - 1) * ax.n_in - 1;
+                    const float x = fmaf(wx.w, __ldg(r + 3) - zref, fmaf(wx.z, __ldg(r + 2) - zref,
+                                    fmaf(wx.y, __ldg(r + 1) - zref, wx.x * (__ldg(r) - zref))));
+                    cub = fmaf(wyv[b], x, cub);
+                }
+                if (cub == cub) f = cub;                           // NaN: one of the 16 neighbours is NaN
+            }
+            f += zref;
+        }
+        out[(size_t)I * ax.n_out + J] = f;
+    }
+}
+
+}  // namespace
+
+int launch_catmull_rom(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
+                       cudaStream_t stream)
+{
+    const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
+    constexpr int CPT = 4, TH = 32, TW = CPT * kThreads;
+    const long long fw = footprint_bound(ax, TW) + 2, fh = footprint_bound(ay, TH) + 2;
+    const long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
+    if (smem <= 160 * 1024 && (out.ny + TH - 1) / TH <= 65535) {
+        static bool attr_set = false;
+        if (!attr_set) {
+            BATHY_CUDA_TRY(cudaFuncSetAttribute(catmull_rom_tiled_kernel<CPT, TH>,
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+            attr_set = true;
+        }
+        dim3 grid((out.nx + TW - 1) / TW, (out.ny + TH - 1) / TH);
+        catmull_rom_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay);
+    } else {
+        dim3 grid((out.nx + kThreads - 1) / kThreads, out.ny < 65535 ? out.ny : 65535);
+        catmull_rom_gather_kernel<<<grid, kThreads, 0, stream>>>(d_in, d_out, ax, ay);
+    }
+    count_launch();
+    return launch_status();
+}
+
+}  // namespace bathy
