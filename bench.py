@@ -168,6 +168,7 @@ def run_ours(args):
     z_in = torch.from_numpy(gw.z).to(dev)
     out_b = torch.empty(go.shape, dtype=torch.float32, device=dev)
     out_s = torch.empty(go.shape, dtype=torch.float32, device=dev)
+    out_c = torch.empty(go.shape, dtype=torch.float32, device=dev)
     ws = torch.empty(B.interp_spline_workspace_bytes(gi, go), dtype=torch.uint8, device=dev)
     sx, sy, sz = (torch.from_numpy(a).to(dev) for a in (sw.x, sw.y, sw.z))
     out_k = torch.empty(gk.shape, dtype=torch.float32, device=dev)
@@ -223,6 +224,18 @@ def run_ours(args):
         [total_ms] + seg.mean(axis=0).tolist(), dist, dev)          # max over ranks
     ms_per_step = total_ms / args.steps
 
+    # ---- NEXT-1: the paper's own Catmull-Rom cubic, timed beside the step (not part of `value`)
+    ec = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    for _ in range(3):
+        B.interp_catmull_rom(z_in, gi, go, out=out_c)
+    barrier()
+    ec[0].record(stream)
+    for _ in range(args.steps):
+        B.interp_catmull_rom(z_in, gi, go, out=out_c)
+    ec[1].record(stream)
+    barrier()
+    ms_cr = sharding.reduce_step_times([ec[0].elapsed_time(ec[1]) / args.steps], dist, dev)[0]
+
     # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the timed region)
     hz = torch.from_numpy(gw.z).pin_memory()
     hob = torch.empty(go.shape, dtype=torch.float32).pin_memory()
@@ -265,13 +278,17 @@ def run_ours(args):
                    "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_spl * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                 "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid,
                                 "note": "whole call (all its kernels) against the compulsory bytes of the method"}},
+        "catmull_rom": {"nodes_per_s": n_grid / (ms_cr * 1e-3), "ms": ms_cr, "launches": 1, "in_step": False,
+                        "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_cr * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                     "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid,
+                                     "note": "NEXT-1 (paper's own cubic, PAPER.md:L136-L144); timed beside the step, not in `value`"}},
         "krige_build_index": {"soundings_per_s": sw.x.shape[0] / (ms_idx * 1e-3), "ms": ms_idx},
         "kriging": {"nodes_per_s": n_krige / (ms_krg * 1e-3), "ms": ms_krg, "k": sw.k, "launches": len(tiles),
                     "ms_per_launch": ms_krg / len(tiles),
                     "roofline": {"bound": "alu", "achieved": kf * n_krige / (ms_krg * 1e-3) / 1e12, "peak": fp32_peak,
                                  "unit": "TFLOP/s", "flop_per_node": kf}},
     }
-    for m in ("bilinear", "spline", "kriging"):
+    for m in ("bilinear", "spline", "kriging", "catmull_rom"):
         r = meth[m]["roofline"]
         r["frac"] = r["achieved"] / r["peak"]
     dom = max(("bilinear", "spline", "kriging"), key=lambda m: meth[m]["ms"])

@@ -29,7 +29,7 @@ __device__ __forceinline__ float4 cr_weights(float t)
 }
 
 template <int CPT, int TH>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 3)
 catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay)
 {
     constexpr int TW = CPT * kThreads;
