@@ -110,24 +110,40 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
-    // x cubic X and x lerp L of footprint row fr at this thread's columns (on sample - z_ref)
+    // x cubic X and x lerp L of input row jrow at this thread's columns, on (sample - z_ref).  With
+    // w1 = 1 - w0 - w2 - w3 the cubic is P1 + w0 (P0 - P1) + w2 (P2 - P1) + w3 (P3 - P1): differences of
+    // neighbouring samples, no weight ever multiplies a 5000 m depth.
+    static_assert(CPT == 4, "column pairs are written out for CPT = 4");
     auto row_eval = [&](int jrow, float* X, float* L) {
         const bool in_grid = jrow >= 0 && jrow <= ay.n_in - 1;
         const float* row = s_tile + (min(max(jrow, fj0), fj1) - fj0) * pitch;
 #pragma unroll
         for (int e = 0; e < CPT; ++e) {
-            const float p0 = row[c0[e]] - zref, p1 = row[c1[e]] - zref, p2 = row[c2[e]] - zref, p3 = row[c3[e]] - zref;
-            const float x = fmaf(cw[e].w, p3, fmaf(cw[e].z, p2, fmaf(cw[e].y, p1, cw[e].x * p0)));
+            const float p1 = row[c1[e]];
+            const float d0 = row[c0[e]] - p1, d2 = row[c2[e]] - p1, d3 = row[c3[e]] - p1, p1z = p1 - zref;
+            const float x = fmaf(cw[e].w, d3, fmaf(cw[e].z, d2, fmaf(cw[e].x, d0, p1z)));
             X[e] = (in_grid && c4ok[e]) ? x : qnan;   // NaN marks "one of the row's 4 neighbours is missing"
-            L[e] = fmaf(ct[e], p2 - p1, p1);
+            L[e] = fmaf(ct[e], d2, p1z);
         }
     };
 
-    float X[4][CPT], L[4][CPT];                       // rows j-1 .. j+2
+    float X[4][CPT], L[4][CPT];                       // rows j-1 .. j+2 (L of row j-1 is never used)
 #pragma unroll
     for (int b = 0; b < 4; ++b)
 #pragma unroll
         for (int e = 0; e < CPT; ++e) X[b][e] = L[b][e] = 0.0f;
+    // what a node of the current row interval evaluates, two columns to a register pair:
+    //   out = wy . Xu + (Lu1 + s Ld) + zc,  where a column that can use the cubic has Lu1 = Ld = 0 and a
+    //   column that falls back to bilinear has Xu = 0 (the choice is per column and interval, not per node:
+    //   the cubic is NaN exactly when one of the 16 neighbours is missing, whatever the y weights)
+    u64 Xu[4][CPT / 2], Lu1[CPT / 2], Ld[CPT / 2];
+    const u64 zc2[CPT / 2] = {pack2(zref + cnan[0], zref + cnan[1]), pack2(zref + cnan[2], zref + cnan[3])};
+#pragma unroll
+    for (int p = 0; p < CPT / 2; ++p) {
+        Lu1[p] = Ld[p] = pack2(0.0f, 0.0f);
+#pragma unroll
+        for (int b = 0; b < 4; ++b) Xu[b][p] = pack2(0.0f, 0.0f);
+    }
     int cur_j = -5;
     float* orow = out + (size_t)I0 * ax.n_out + Jt;
     for (int r = 0; r < nrows; ++r, orow += ax.n_out) {
@@ -149,17 +165,38 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
 #pragma unroll
                 for (int b = 0; b < 4; ++b) row_eval(j - 1 + b, X[b], L[b]);
             }
+            float xu[4][CPT], l1[CPT], ld[CPT];
+#pragma unroll
+            for (int e = 0; e < CPT; ++e) {
+                const float sum = (X[0][e] + X[1][e]) + (X[2][e] + X[3][e]);
+                const bool use = sum == sum;           // no NaN among the 4 row cubics
+#pragma unroll
+                for (int b = 0; b < 4; ++b) xu[b][e] = use ? X[b][e] : 0.0f;
+                l1[e] = use ? 0.0f : L[1][e];
+                ld[e] = use ? 0.0f : L[2][e] - L[1][e];
+            }
+#pragma unroll
+            for (int p = 0; p < CPT / 2; ++p) {
+#pragma unroll
+                for (int b = 0; b < 4; ++b) Xu[b][p] = pack2(xu[b][2 * p], xu[b][2 * p + 1]);
+                Lu1[p] = pack2(l1[2 * p], l1[2 * p + 1]);
+                Ld[p] = pack2(ld[2 * p], ld[2 * p + 1]);
+            }
             cur_j = j;
         }
         const float s = __int_as_float(rw.y);
         const float4 wy = s_wy[r];
+        const u64 s2 = pack2(s, s), w0 = pack2(wy.x, wy.x), w1 = pack2(wy.y, wy.y), w2 = pack2(wy.z, wy.z), w3 = pack2(wy.w, wy.w);
 #pragma unroll
-        for (int e = 0; e < CPT; ++e) {
-            const float cub = fmaf(wy.w, X[3][e], fmaf(wy.z, X[2][e], fmaf(wy.y, X[1][e], wy.x * X[0][e])));
-            const float bil = fmaf(s, L[2][e] - L[1][e], L[1][e]);
-            // cub is NaN exactly when one of the 16 neighbours is outside the grid or NaN (0 * NaN = NaN)
-            const float v = ((cub == cub) ? cub : bil) + zref + cnan[e];
-            if (cok[e]) orow[32 * e] = v;
+        for (int p = 0; p < CPT / 2; ++p) {
+            u64 o = ffma2(s2, Ld[p], Lu1[p]);
+            o = ffma2(w0, Xu[0][p], o);
+            o = ffma2(w1, Xu[1][p], o);
+            o = ffma2(w2, Xu[2][p], o);
+            o = ffma2(w3, Xu[3][p], o);
+            o = fadd2(o, zc2[p]);
+            if (cok[2 * p]) orow[64 * p] = lo_of(o);
+            if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
         }
     }
 }
