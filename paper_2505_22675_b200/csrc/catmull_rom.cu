@@ -110,40 +110,54 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
-    // x cubic X and x lerp L of input row jrow at this thread's columns, on (sample - z_ref).  With
+    // x cubic of input row jrow at this thread's columns, on (sample - z_ref), two columns to a pair.  With
     // w1 = 1 - w0 - w2 - w3 the cubic is P1 + w0 (P0 - P1) + w2 (P2 - P1) + w3 (P3 - P1): differences of
-    // neighbouring samples, no weight ever multiplies a 5000 m depth.
+    // neighbouring samples, no weight ever multiplies a 5000 m depth.  A column that lacks one of its 4 x
+    // neighbours subtracts NaN instead of z_ref, a row outside the grid is NaN: X is NaN exactly when one
+    // of the row's 4 neighbours is missing.
     static_assert(CPT == 4, "column pairs are written out for CPT = 4");
-    auto row_eval = [&](int jrow, float* X, float* L) {
-        const bool in_grid = jrow >= 0 && jrow <= ay.n_in - 1;
-        const float* row = s_tile + (min(max(jrow, fj0), fj1) - fj0) * pitch;
+    float zrc[CPT];
+#pragma unroll
+    for (int e = 0; e < CPT; ++e) zrc[e] = c4ok[e] ? zref : qnan;
+    auto row_eval = [&](int jrow, u64* X2) {
+        if (jrow < 0 || jrow > ay.n_in - 1) {          // CTA-uniform
+            X2[0] = X2[1] = pack2(qnan, qnan);
+            return;
+        }
+        const float* row = s_tile + (jrow - fj0) * pitch;
+        float x[CPT];
 #pragma unroll
         for (int e = 0; e < CPT; ++e) {
             const float p1 = row[c1[e]];
-            const float d0 = row[c0[e]] - p1, d2 = row[c2[e]] - p1, d3 = row[c3[e]] - p1, p1z = p1 - zref;
-            const float x = fmaf(cw[e].w, d3, fmaf(cw[e].z, d2, fmaf(cw[e].x, d0, p1z)));
-            X[e] = (in_grid && c4ok[e]) ? x : qnan;   // NaN marks "one of the row's 4 neighbours is missing"
-            L[e] = fmaf(ct[e], d2, p1z);
+            const float d0 = row[c0[e]] - p1, d2 = row[c2[e]] - p1, d3 = row[c3[e]] - p1;
+            x[e] = fmaf(cw[e].w, d3, fmaf(cw[e].z, d2, fmaf(cw[e].x, d0, p1 - zrc[e])));
+        }
+        X2[0] = pack2(x[0], x[1]); X2[1] = pack2(x[2], x[3]);
+    };
+    // x lerp of input row jrow (always inside the grid) for the bilinear fallback
+    auto row_lerp = [&](int jrow, float* L) {
+        const float* row = s_tile + (jrow - fj0) * pitch;
+#pragma unroll
+        for (int e = 0; e < CPT; ++e) {
+            const float p1 = row[c1[e]];
+            L[e] = fmaf(ct[e], row[c2[e]] - p1, p1 - zref);
         }
     };
 
-    float X[4][CPT], L[4][CPT];                       // rows j-1 .. j+2 (L of row j-1 is never used)
-#pragma unroll
-    for (int b = 0; b < 4; ++b)
-#pragma unroll
-        for (int e = 0; e < CPT; ++e) X[b][e] = L[b][e] = 0.0f;
-    // what a node of the current row interval evaluates, two columns to a register pair:
-    //   out = wy . Xu + (Lu1 + s Ld) + zc,  where a column that can use the cubic has Lu1 = Ld = 0 and a
-    //   column that falls back to bilinear has Xu = 0 (the choice is per column and interval, not per node:
-    //   the cubic is NaN exactly when one of the 16 neighbours is missing, whatever the y weights)
+    u64 X[4][CPT / 2];                                // x cubics of rows j-1 .. j+2
+    // what a node of the current row interval evaluates:  out = wy . Xu + (Lu1 + s Ld) + zc, where a column
+    // that can use the cubic has Lu1 = Ld = 0 and a column that falls back to bilinear has Xu = 0 (the choice
+    // is per column and interval, not per node: the cubic is NaN exactly when one of the 16 neighbours is
+    // missing, whatever the y weights).  `plain`: every column of the warp uses the cubic (the usual case).
     u64 Xu[4][CPT / 2], Lu1[CPT / 2], Ld[CPT / 2];
     const u64 zc2[CPT / 2] = {pack2(zref + cnan[0], zref + cnan[1]), pack2(zref + cnan[2], zref + cnan[3])};
 #pragma unroll
     for (int p = 0; p < CPT / 2; ++p) {
         Lu1[p] = Ld[p] = pack2(0.0f, 0.0f);
 #pragma unroll
-        for (int b = 0; b < 4; ++b) Xu[b][p] = pack2(0.0f, 0.0f);
+        for (int b = 0; b < 4; ++b) X[b][p] = Xu[b][p] = pack2(0.0f, 0.0f);
     }
+    bool plain = true;
     int cur_j = -5;
     float* orow = out + (size_t)I0 * ax.n_out + Jt;
     for (int r = 0; r < nrows; ++r, orow += ax.n_out) {
@@ -157,46 +171,61 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         if (j != cur_j) {                              // CTA-uniform: the window of 4 input rows moves
             if (j == cur_j + 1) {
 #pragma unroll
-                for (int b = 0; b < 3; ++b)
-#pragma unroll
-                    for (int e = 0; e < CPT; ++e) { X[b][e] = X[b + 1][e]; L[b][e] = L[b + 1][e]; }
-                row_eval(j + 2, X[3], L[3]);
+                for (int b = 0; b < 3; ++b) { X[b][0] = X[b + 1][0]; X[b][1] = X[b + 1][1]; }
+                row_eval(j + 2, X[3]);
             } else {
 #pragma unroll
-                for (int b = 0; b < 4; ++b) row_eval(j - 1 + b, X[b], L[b]);
-            }
-            float xu[4][CPT], l1[CPT], ld[CPT];
-#pragma unroll
-            for (int e = 0; e < CPT; ++e) {
-                const float sum = (X[0][e] + X[1][e]) + (X[2][e] + X[3][e]);
-                const bool use = sum == sum;           // no NaN among the 4 row cubics
-#pragma unroll
-                for (int b = 0; b < 4; ++b) xu[b][e] = use ? X[b][e] : 0.0f;
-                l1[e] = use ? 0.0f : L[1][e];
-                ld[e] = use ? 0.0f : L[2][e] - L[1][e];
-            }
-#pragma unroll
-            for (int p = 0; p < CPT / 2; ++p) {
-#pragma unroll
-                for (int b = 0; b < 4; ++b) Xu[b][p] = pack2(xu[b][2 * p], xu[b][2 * p + 1]);
-                Lu1[p] = pack2(l1[2 * p], l1[2 * p + 1]);
-                Ld[p] = pack2(ld[2 * p], ld[2 * p + 1]);
+                for (int b = 0; b < 4; ++b) row_eval(j - 1 + b, X[b]);
             }
             cur_j = j;
-        }
-        const float s = __int_as_float(rw.y);
-        const float4 wy = s_wy[r];
-        const u64 s2 = pack2(s, s), w0 = pack2(wy.x, wy.x), w1 = pack2(wy.y, wy.y), w2 = pack2(wy.z, wy.z), w3 = pack2(wy.w, wy.w);
+            const u64 sum0 = fadd2(fadd2(X[0][0], X[1][0]), fadd2(X[2][0], X[3][0]));
+            const u64 sum1 = fadd2(fadd2(X[0][1], X[1][1]), fadd2(X[2][1], X[3][1]));
+            const float sm[CPT] = {lo_of(sum0), hi_of(sum0), lo_of(sum1), hi_of(sum1)};
+            bool use[CPT];
 #pragma unroll
-        for (int p = 0; p < CPT / 2; ++p) {
-            u64 o = ffma2(s2, Ld[p], Lu1[p]);
-            o = ffma2(w0, Xu[0][p], o);
-            o = ffma2(w1, Xu[1][p], o);
-            o = ffma2(w2, Xu[2][p], o);
-            o = ffma2(w3, Xu[3][p], o);
-            o = fadd2(o, zc2[p]);
-            if (cok[2 * p]) orow[64 * p] = lo_of(o);
-            if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
+            for (int e = 0; e < CPT; ++e) use[e] = sm[e] == sm[e];      // no NaN among the 4 row cubics
+            plain = __all_sync(0xffffffffu, use[0] && use[1] && use[2] && use[3]);
+            if (!plain) {                              // somewhere in the warp a column falls back to bilinear
+                float l1[CPT], l2[CPT];
+                row_lerp(j, l1);
+                row_lerp(j + 1, l2);
+#pragma unroll
+                for (int p = 0; p < CPT / 2; ++p) {
+                    const bool ua = use[2 * p], ub = use[2 * p + 1];
+#pragma unroll
+                    for (int b = 0; b < 4; ++b)
+                        Xu[b][p] = pack2(ua ? lo_of(X[b][p]) : 0.0f, ub ? hi_of(X[b][p]) : 0.0f);
+                    Lu1[p] = pack2(ua ? 0.0f : l1[2 * p], ub ? 0.0f : l1[2 * p + 1]);
+                    Ld[p] = pack2(ua ? 0.0f : l2[2 * p] - l1[2 * p], ub ? 0.0f : l2[2 * p + 1] - l1[2 * p + 1]);
+                }
+            }
+        }
+        const float4 wy = s_wy[r];
+        const u64 w0 = pack2(wy.x, wy.x), w1 = pack2(wy.y, wy.y), w2 = pack2(wy.z, wy.z), w3 = pack2(wy.w, wy.w);
+        if (plain) {
+#pragma unroll
+            for (int p = 0; p < CPT / 2; ++p) {
+                u64 o = ffma2(w1, X[1][p], fmul2(w0, X[0][p]));
+                o = ffma2(w2, X[2][p], o);
+                o = ffma2(w3, X[3][p], o);
+                o = fadd2(o, zc2[p]);
+                if (cok[2 * p]) orow[64 * p] = lo_of(o);
+                if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
+            }
+        } else {
+            const float s = __int_as_float(rw.y);
+            const u64 s2 = pack2(s, s);
+#pragma unroll
+            for (int p = 0; p < CPT / 2; ++p) {
+                u64 o = ffma2(s2, Ld[p], Lu1[p]);
+                o = ffma2(w0, Xu[0][p], o);
+                o = ffma2(w1, Xu[1][p], o);
+                o = ffma2(w2, Xu[2][p], o);
+                o = ffma2(w3, Xu[3][p], o);
+                o = fadd2(o, zc2[p]);
+                if (cok[2 * p]) orow[64 * p] = lo_of(o);
+                if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
+            }
         }
     }
 }
