@@ -89,8 +89,9 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     const int Jt = J0 + warp * (32 * CPT) + lane;     // column of e = 0
     bool cok[CPT], c4ok[CPT];                         // column inside the tile / has its 4 x neighbours in the grid
     float ct[CPT], cnan[CPT];
-    float4 cw[CPT];
-    int c0[CPT], c1[CPT], c2[CPT], c3[CPT];           // offsets of P0..P3 in a footprint row (clamped into it)
+    float cw0[CPT], cw2[CPT], cw3[CPT];               // x weights of P0, P2, P3 (P1's is 1 minus their sum)
+    int c1[CPT], cl[CPT], cr[CPT];                    // offset of P1 in a footprint row; P0 at c1 - cl, P3 at c1 + 1 + cr
+                                                      // (cl, cr in {0, 1}: clamped into the footprint)
     const float qnan = __int_as_float(0x7fc00000);
 #pragma unroll
     for (int e = 0; e < CPT; ++e) {
@@ -101,11 +102,11 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         cnan[e] = (i < 0) ? qnan : 0.0f;
         const int ic = (i < 0) ? fi0 : i;             // a column outside the extent still reads inside the footprint
         c4ok[e] = (i >= 1) && (i + 2 <= ax.n_in - 1);
-        cw[e] = cr_weights(ct[e]);
+        const float4 w = cr_weights(ct[e]);
+        cw0[e] = w.x; cw2[e] = w.z; cw3[e] = w.w;
         c1[e] = min(max(ic, fi0), fi1 - 1) - fi0 + offx;
-        c2[e] = c1[e] + 1;
-        c0[e] = max(c1[e] - 1, offx);
-        c3[e] = min(c1[e] + 2, fi1 - fi0 + offx);
+        cl[e] = (c1[e] - 1 >= offx) ? 1 : 0;
+        cr[e] = (c1[e] + 2 <= fi1 - fi0 + offx) ? 1 : 0;
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
@@ -128,9 +129,10 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         float x[CPT];
 #pragma unroll
         for (int e = 0; e < CPT; ++e) {
-            const float p1 = row[c1[e]];
-            const float d0 = row[c0[e]] - p1, d2 = row[c2[e]] - p1, d3 = row[c3[e]] - p1;
-            x[e] = fmaf(cw[e].w, d3, fmaf(cw[e].z, d2, fmaf(cw[e].x, d0, p1 - zrc[e])));
+            const float* q = row + c1[e];
+            const float p1 = q[0];
+            const float d0 = q[-cl[e]] - p1, d2 = q[1] - p1, d3 = q[1 + cr[e]] - p1;
+            x[e] = fmaf(cw3[e], d3, fmaf(cw2[e], d2, fmaf(cw0[e], d0, p1 - zrc[e])));
         }
         X2[0] = pack2(x[0], x[1]); X2[1] = pack2(x[2], x[3]);
     };
@@ -140,7 +142,7 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
 #pragma unroll
         for (int e = 0; e < CPT; ++e) {
             const float p1 = row[c1[e]];
-            L[e] = fmaf(ct[e], row[c2[e]] - p1, p1 - zref);
+            L[e] = fmaf(ct[e], row[c1[e] + 1] - p1, p1 - zref);
         }
     };
 
