@@ -120,21 +120,32 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     float zrc[CPT];
 #pragma unroll
     for (int e = 0; e < CPT; ++e) zrc[e] = c4ok[e] ? zref : qnan;
-    auto row_eval = [&](int jrow, u64* X2) {
+    const u64 w0x[CPT / 2] = {pack2(cw0[0], cw0[1]), pack2(cw0[2], cw0[3])};
+    const u64 w2x[CPT / 2] = {pack2(cw2[0], cw2[1]), pack2(cw2[2], cw2[3])};
+    const u64 w3x[CPT / 2] = {pack2(cw3[0], cw3[1]), pack2(cw3[2], cw3[3])};
+    const u64 nzr[CPT / 2] = {pack2(-zrc[0], -zrc[1]), pack2(-zrc[2], -zrc[3])};
+    const u64 neg1 = pack2(-1.0f, -1.0f);
+    // returns true (warp-uniform) when some column of the warp got a NaN in this row
+    auto row_eval = [&](int jrow, u64* X2) -> bool {
         if (jrow < 0 || jrow > ay.n_in - 1) {          // CTA-uniform
             X2[0] = X2[1] = pack2(qnan, qnan);
-            return;
+            return true;
         }
         const float* row = s_tile + (jrow - fj0) * pitch;
-        float x[CPT];
 #pragma unroll
-        for (int e = 0; e < CPT; ++e) {
-            const float* q = row + c1[e];
-            const float p1 = q[0];
-            const float d0 = q[-cl[e]] - p1, d2 = q[1] - p1, d3 = q[1 + cr[e]] - p1;
-            x[e] = fmaf(cw3[e], d3, fmaf(cw2[e], d2, fmaf(cw0[e], d0, p1 - zrc[e])));
+        for (int p = 0; p < CPT / 2; ++p) {
+            const float* qa = row + c1[2 * p];
+            const float* qb = row + c1[2 * p + 1];
+            const u64 p1 = pack2(qa[0], qb[0]);
+            const u64 np1 = fmul2(p1, neg1);
+            const u64 d0 = fadd2(pack2(qa[-cl[2 * p]], qb[-cl[2 * p + 1]]), np1);
+            const u64 d2 = fadd2(pack2(qa[1], qb[1]), np1);
+            const u64 d3 = fadd2(pack2(qa[1 + cr[2 * p]], qb[1 + cr[2 * p + 1]]), np1);
+            X2[p] = ffma2(w3x[p], d3, ffma2(w2x[p], d2, ffma2(w0x[p], d0, fadd2(p1, nzr[p]))));
         }
-        X2[0] = pack2(x[0], x[1]); X2[1] = pack2(x[2], x[3]);
+        const u64 t = fadd2(X2[0], X2[1]);
+        const float u = lo_of(t) + hi_of(t);
+        return __any_sync(0xffffffffu, u != u);
     };
     // x lerp of input row jrow (always inside the grid) for the bilinear fallback
     auto row_lerp = [&](int jrow, float* L) {
@@ -160,6 +171,7 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         for (int b = 0; b < 4; ++b) X[b][p] = Xu[b][p] = pack2(0.0f, 0.0f);
     }
     bool plain = true;
+    bool bad[4] = {true, true, true, true};           // warp-uniform: row b of the window has a NaN somewhere in the warp
     int cur_j = -5;
     float* orow = out + (size_t)I0 * ax.n_out + Jt;
     for (int r = 0; r < nrows; ++r, orow += ax.n_out) {
@@ -173,21 +185,21 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         if (j != cur_j) {                              // CTA-uniform: the window of 4 input rows moves
             if (j == cur_j + 1) {
 #pragma unroll
-                for (int b = 0; b < 3; ++b) { X[b][0] = X[b + 1][0]; X[b][1] = X[b + 1][1]; }
-                row_eval(j + 2, X[3]);
+                for (int b = 0; b < 3; ++b) { X[b][0] = X[b + 1][0]; X[b][1] = X[b + 1][1]; bad[b] = bad[b + 1]; }
+                bad[3] = row_eval(j + 2, X[3]);
             } else {
 #pragma unroll
-                for (int b = 0; b < 4; ++b) row_eval(j - 1 + b, X[b]);
+                for (int b = 0; b < 4; ++b) bad[b] = row_eval(j - 1 + b, X[b]);
             }
             cur_j = j;
-            const u64 sum0 = fadd2(fadd2(X[0][0], X[1][0]), fadd2(X[2][0], X[3][0]));
-            const u64 sum1 = fadd2(fadd2(X[0][1], X[1][1]), fadd2(X[2][1], X[3][1]));
-            const float sm[CPT] = {lo_of(sum0), hi_of(sum0), lo_of(sum1), hi_of(sum1)};
-            bool use[CPT];
-#pragma unroll
-            for (int e = 0; e < CPT; ++e) use[e] = sm[e] == sm[e];      // no NaN among the 4 row cubics
-            plain = __all_sync(0xffffffffu, use[0] && use[1] && use[2] && use[3]);
+            plain = !(bad[0] || bad[1] || bad[2] || bad[3]);
             if (!plain) {                              // somewhere in the warp a column falls back to bilinear
+                const u64 sum0 = fadd2(fadd2(X[0][0], X[1][0]), fadd2(X[2][0], X[3][0]));
+                const u64 sum1 = fadd2(fadd2(X[0][1], X[1][1]), fadd2(X[2][1], X[3][1]));
+                const float sm[CPT] = {lo_of(sum0), hi_of(sum0), lo_of(sum1), hi_of(sum1)};
+                bool use[CPT];
+#pragma unroll
+                for (int e = 0; e < CPT; ++e) use[e] = sm[e] == sm[e];  // no NaN among the column's 4 row cubics
                 float l1[CPT], l2[CPT];
                 row_lerp(j, l1);
                 row_lerp(j + 1, l2);
