@@ -329,10 +329,15 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
             const u64 cn2[2] = {pack2(cnan[0], cnan[1]), pack2(cnan[2], cnan[3])};
             const bool full = !oob_rows && (Jp + 128 <= Jend);        // warp-uniform
             int curk = -2;
+            // (rolled: the unrolled form is several thousand instructions, more than the instruction cache
+            // holds for 16 warps at different places; lane i keeps rsv[i])
+            int rsv_lane = rsv[0];
 #pragma unroll
+            for (int i = 1; i <= TI; ++i) rsv_lane = (lane == i) ? rsv[i] : rsv_lane;
+#pragma unroll 1
             for (int ki = 0; ki < TI; ++ki) {
                 const int kj = kja + ki;
-                const int rs = rsv[ki], re = rsv[ki + 1];
+                const int rs = __shfl_sync(0xffffffffu, rsv_lane, ki), re = __shfl_sync(0xffffffffu, rsv_lane, ki + 1);
                 if (kj >= kjb || rs >= re) continue;   // no such row of cells / no output row in it
                 if (kj == curk + 1) {
 #pragma unroll
