@@ -249,13 +249,14 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
             if (lane < nky) {
                 const int plane = warp & 1, half = warp >> 1;
                 const float* row = (plane == 0 ? s_zf : s_my) + lane * PZ + (half ? WX - HW : 0);
-                float2* dst = reinterpret_cast<float2*>(s_q + lane * PQ + (half ? HL : 0)) + plane;
+                static_assert(WX - HW == HL - 1 && NXI - HL == HL - 1, "the halves share one instantiation");
+                float2* dst = reinterpret_cast<float2*>(s_q + lane * PQ + (half ? HL - 1 : 0)) + plane;
                 auto rd = [&](int q) { return row[q]; };
-                auto st = [&](int k, float v, float m) { dst[2 * k] = make_float2(v, m); };
                 // left: window knots [0, HW), kept = tile knots [0, HL) = window [H, H + HL)
-                // right: window knots [WX - HW, WX), kept = tile knots [HL, NXI) = window [HW - H - (NXI - HL), HW - H)
-                if (half == 0) thomas_window<HW, true, H, HL>(rd, st, 0, 0);
-                else           thomas_window<HW, true, HW - H - (NXI - HL), NXI - HL>(rd, st, 0, 0);
+                // right: window knots [WX - HW, WX), window [H, H + HL) = tile knots [HL - 1, NXI): the same
+                // code (one instantiation, half the instructions); its first knot is the left half's last
+                auto st = [&](int k, float v, float m) { if (k > 0 || half == 0) dst[2 * k] = make_float2(v, m); };
+                thomas_window<HW, true, H, HL>(rd, st, 0, 0);
             }
         } else if (warp < 2 && lane < nky) {
             const float* row = (warp == 0 ? s_zf : s_my) + lane * PZ;
@@ -291,7 +292,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         __syncwarp();
         for (int Jp = Jbeg; Jp < Jend; Jp += 128) {
             const int Jt = Jp + lane;                  // column of e = 0; e-th column is 32 e further
-            if (Jt >= Jend) continue;
+            // (a lane past the tile's last column stays: the interval loop below shuffles over the full warp)
             bool cok[4];
             u64 wl[4], wh[4];                          // blending weights (1-t, C(t)) and (t, D(t)) of the column
             float cnan[4];
