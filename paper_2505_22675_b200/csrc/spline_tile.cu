@@ -105,12 +105,13 @@ __device__ __forceinline__ void thomas_window(Rd rd, St st, int k0_rt, int nk_rt
 
 // Per-axis tables of the output->input map, computed once per call in float64 exactly as the
 // definition (readings B1/B2) so that the tile kernel does no double-precision arithmetic:
-//   tab[n]    = (interval index or -1 as int bits, t, C(t) = ((1-t)^2 - 1)(1-t), D(t) = (t^2 - 1) t)
+//   rowtab[n] = (interval index or -1 as int bits, t, C(t) = ((1-t)^2 - 1)(1-t), D(t) = (t^2 - 1) t)
+//   colw[n]   = (1-t, C(t), t, D(t)), coli[n] = interval index or -1
 //   tb[b]     = first output node whose (clamped) interval is >= b * tile cells; tb[nb] = n_out
 //   rfirst[j] = first output row whose (clamped) interval is >= j, j = 0 .. ny_in.
 __global__ void __launch_bounds__(256)
-spline_tables_kernel(AxisMap ax, AxisMap ay, float4* __restrict__ coltab, float4* __restrict__ rowtab,
-                     int* __restrict__ tbx, int* __restrict__ tby, int* __restrict__ rfirst,
+spline_tables_kernel(AxisMap ax, AxisMap ay, float4* __restrict__ colw, float4* __restrict__ rowtab,
+                     int* __restrict__ tbx, int* __restrict__ tby, int* __restrict__ rfirst, int* __restrict__ coli,
                      int nbx, int nby, int txi, int tyi)
 {
     int n = blockIdx.x * 256 + threadIdx.x;
@@ -121,7 +122,16 @@ spline_tables_kernel(AxisMap ax, AxisMap ay, float4* __restrict__ coltab, float4
         float t;
         const int i = axis_locate(m, J, &t);
         const float a = 1.0f - t;
-        (isx ? coltab : rowtab)[J] = make_float4(__int_as_float(i), t, (a * a - 1.0f) * a, (t * t - 1.0f) * t);
+        const float C = (a * a - 1.0f) * a, D = (t * t - 1.0f) * t;
+        if (isx) {
+            // columns: the blending weights as two fp32x2 operands (1-t, C), (t, D), NaN outside the input
+            // extent (reading B4: the node then comes out NaN without a test in the tile kernel)
+            const float qn = __int_as_float(0x7fc00000);
+            colw[J] = (i < 0) ? make_float4(qn, qn, qn, qn) : make_float4(a, C, t, D);
+            coli[J] = i;
+        } else {
+            rowtab[J] = make_float4(__int_as_float(i), t, C, D);
+        }
         return;
     }
     n -= ax.n_out + ay.n_out;
@@ -135,9 +145,9 @@ spline_tables_kernel(AxisMap ax, AxisMap ay, float4* __restrict__ coltab, float4
 template <class S>
 __global__ void __launch_bounds__(kTileThreads, 4)
 spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay,
-                   const float4* __restrict__ coltab, const float4* __restrict__ rowtab,
+                   const float4* __restrict__ colw, const float4* __restrict__ rowtab,
                    const int* __restrict__ tbx, const int* __restrict__ tby, const int* __restrict__ rfirst,
-                   int nbx, int n_tiles, int pf_dist)
+                   const int* __restrict__ coli, int nbx, int n_tiles, int pf_dist)
 {
     constexpr int TXI = S::TXI, TYI = S::TYI, H = S::H, WX = S::WX, WY = S::WY;
     constexpr int NXI = S::NXI, NYI = S::NYI, PZ = S::PZ, PA = S::PA, PQ = S::PQ;
@@ -295,18 +305,17 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
             // (a lane past the tile's last column stays: the interval loop below shuffles over the full warp)
             bool cok[4];
             u64 wl[4], wh[4];                          // blending weights (1-t, C(t)) and (t, D(t)) of the column
-            float cnan[4];
             const float4* qc[4];                       // left knot record of the column's interval, knot row 0 of the tile
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const int J = Jt + 32 * e;
                 cok[e] = J < Jend;
-                const float4 ct = cok[e] ? __ldg(coltab + J) : make_float4(__int_as_float(-1), 0.0f, 0.0f, 0.0f);
-                const int i = __float_as_int(ct.x);
-                wl[e] = pack2(1.0f - ct.y, ct.z);
-                wh[e] = pack2(ct.y, ct.w);
-                cnan[e] = (i < 0 && cok[e]) ? qnan : 0.0f;   // outside the input extent
-                qc[e] = s_q + ((i < 0) ? 0 : i - i0);
+                // the weights arrive as 64-bit pairs (NaN pairs outside the input extent): no repacking
+                const ulonglong2 cw = cok[e] ? __ldg(reinterpret_cast<const ulonglong2*>(colw + J)) : make_ulonglong2(0ull, 0ull);
+                const int i = cok[e] ? __ldg(coli + J) : -1;
+                wl[e] = cw.x;
+                wh[e] = cw.y;
+                qc[e] = s_q + max(i - i0, 0);
             }
             // x-direction splines of knot row kj at this thread's 4 columns, paired by column:
             // X2[p] = (X[2p], X[2p+1])
@@ -327,7 +336,6 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
             u64 X0[2], X1[2], Xd[2], Y0[2], Y1[2];
 #pragma unroll
             for (int p = 0; p < 2; ++p) X0[p] = X1[p] = Xd[p] = Y0[p] = Y1[p] = pack2(0.0f, 0.0f);
-            const u64 cn2[2] = {pack2(cnan[0], cnan[1]), pack2(cnan[2], cnan[3])};
             const bool full = !oob_rows && (Jp + 128 <= Jend);        // warp-uniform
             int curk = -2;
             // (rolled: the unrolled form is several thousand instructions, more than the instruction cache
@@ -348,10 +356,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 }
                 knot_row(kj + 1, X1, Y1);
 #pragma unroll
-                for (int p = 0; p < 2; ++p) {
-                    Xd[p] = ffma2(X0[p], neg1, X1[p]);
-                    X0[p] = fadd2(X0[p], cn2[p]);
-                }
+                for (int p = 0; p < 2; ++p) Xd[p] = ffma2(X0[p], neg1, X1[p]);
                 curk = kj;
                 float* op = out + (size_t)rs * ax.n_out + Jt;
                 if (full) {                            // all four columns inside the tile, no row outside the extent
@@ -401,18 +406,19 @@ int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMa
         attr_set = true;
     }
     dim3 grid((ax.n_in - 1 + S::TXI - 1) / S::TXI, (ay.n_in - 1 + S::TYI - 1) / S::TYI);
-    float4* coltab = static_cast<float4*>(d_ws);
-    float4* rowtab = coltab + ax.n_out;
+    float4* colw = static_cast<float4*>(d_ws);
+    float4* rowtab = colw + ax.n_out;
     int* tbx = reinterpret_cast<int*>(rowtab + ay.n_out);
     int* tby = tbx + grid.x + 1;
     int* rfirst = tby + grid.y + 1;
+    int* coli = rfirst + ay.n_in + 1;
     const long long items = (long long)ax.n_out + ay.n_out + grid.x + grid.y + 2 + ay.n_in + 1;
-    spline_tables_kernel<<<(unsigned)((items + 255) / 256), 256, 0, stream>>>(ax, ay, coltab, rowtab, tbx, tby, rfirst,
+    spline_tables_kernel<<<(unsigned)((items + 255) / 256), 256, 0, stream>>>(ax, ay, colw, rowtab, tbx, tby, rfirst, coli,
                                                                               (int)grid.x, (int)grid.y, S::TXI, S::TYI);
     const long long n_tiles = (long long)grid.x * grid.y;
     if (n_tiles > 0x7fffffffLL) return 1;
     const unsigned ctas = (unsigned)n_tiles;
-    spline_tile_kernel<S><<<ctas, kTileThreads, S::smem_bytes, stream>>>(d_in, d_out, ax, ay, coltab, rowtab, tbx, tby, rfirst,
+    spline_tile_kernel<S><<<ctas, kTileThreads, S::smem_bytes, stream>>>(d_in, d_out, ax, ay, colw, rowtab, tbx, tby, rfirst, coli,
                                                                           (int)grid.x, (int)n_tiles, 4 * kSMs /* CTAs resident at once */);
     count_launch(2);
     return launch_status();
@@ -425,7 +431,7 @@ int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMa
 // Bytes of the axis tables at the start of the workspace (an upper bound over both tile shapes).
 size_t spline_tiled_table_bytes(const grid_geom_t& in, const grid_geom_t& out)
 {
-    const size_t b = 16 * ((size_t)out.nx + (size_t)out.ny) + 4 * ((size_t)in.nx + 2 * (size_t)in.ny + 8);
+    const size_t b = 16 * ((size_t)out.nx + (size_t)out.ny) + 4 * ((size_t)in.nx + 2 * (size_t)in.ny + (size_t)out.nx + 8);
     return (b + 255) / 256 * 256;
 }
 
