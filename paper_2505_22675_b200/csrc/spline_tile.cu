@@ -21,6 +21,8 @@
 // All M are stored scaled by h^2/6 (M' = M h^2/6 solves [1 4 1] M' = second difference of z), so
 // the grid spacing drops out of the arithmetic.
 // HBM traffic: the input once (window halos are L2 hits), the output once = the compulsory bytes.
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace bathy {
@@ -227,12 +229,12 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const float* s_z = s_zbuf;
         float zref = __ldg(in + (size_t)w0y * ax.n_in + w0x);
         if (!isfinite(zref)) zref = 0.0f;
-        // the warp's knot intervals and their output rows (rows of interval kj: [rsv[kj-kja], rsv[kj-kja+1]))
+        // the warp's band: knot intervals [kja, kjb) of the tile = output rows [rb, re) (rfirst[j]: first
+        // output row whose interval is >= j)
         constexpr int TI = (TYI + NW - 1) / NW;                           // knot intervals per warp
         const int kja = warp * TI, kjb = min(min(kja + TI, TYI), nky - 1);
-        int rsv[TI + 1];
-#pragma unroll
-        for (int i = 0; i <= TI; ++i) rsv[i] = min(max(__ldg(rfirst + min(j0 + kja + i, ay.n_in)), Ibeg), Iend);
+        const int rb = min(max(__ldg(rfirst + min(j0 + kja, ay.n_in)), Ibeg), Iend);
+        const int re = (kjb > kja) ? min(max(__ldg(rfirst + min(j0 + kjb, ay.n_in)), Ibeg), Iend) : rb;
         asm volatile("cp.async.wait_group 0;" ::: "memory");             // the window has landed
         __syncthreads();
 
@@ -296,16 +298,16 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         // sweeps are dead): a global load per row would expose an L2 round trip in every interval
         constexpr int RT_CAP = (2 * NYI * PZ) / (4 * NW);                 // float4 entries per warp
         float4* s_rt = reinterpret_cast<float4*>(s_zf) + warp * RT_CAP;
-        const int rt0 = rsv[0], rt_n = rsv[TI] - rsv[0];
+        const int rt_n = re - rb;
         const bool rt_ok = rt_n <= RT_CAP;                               // warp-uniform
-        if (rt_ok) for (int i = lane; i < rt_n; i += 32) s_rt[i] = __ldg(rowtab + rt0 + i);
+        if (rt_ok) for (int i = lane; i < rt_n; i += 32) s_rt[i] = __ldg(rowtab + rb + i);
         __syncwarp();
+        const float4* rt_base = rt_ok ? s_rt : rowtab + rb;              // row entry of output row rb
         for (int Jp = Jbeg; Jp < Jend; Jp += 128) {
             const int Jt = Jp + lane;                  // column of e = 0; e-th column is 32 e further
-            // (a lane past the tile's last column stays: the interval loop below shuffles over the full warp)
             bool cok[4];
             u64 wl[4], wh[4];                          // blending weights (1-t, C(t)) and (t, D(t)) of the column
-            const float4* qc[4];                       // left knot record of the column's interval, knot row 0 of the tile
+            unsigned qc[4];                            // left knot record of the column's interval, knot row 0 of the tile
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const int J = Jt + 32 * e;
@@ -315,18 +317,20 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 const int i = cok[e] ? __ldg(coli + J) : -1;
                 wl[e] = cw.x;
                 wh[e] = cw.y;
-                qc[e] = s_q + max(i - i0, 0);
+                qc[e] = (unsigned)__cvta_generic_to_shared(s_q + max(i - i0, 0));
             }
             // x-direction splines of knot row kj at this thread's 4 columns, paired by column:
             // X2[p] = (X[2p], X[2p+1])
             auto knot_row = [&](int kj, u64* X2, u64* Y2) {
                 float xv[4], yv[4];
+                const unsigned ro = (unsigned)(kj * (PQ * 16));
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const ulonglong2 L = *reinterpret_cast<const ulonglong2*>(qc[e] + kj * PQ);       // (z, Mx'), (My', Mxy')
-                    const ulonglong2 R = *reinterpret_cast<const ulonglong2*>(qc[e] + kj * PQ + 1);
-                    const u64 ux = ffma2(R.x, wh[e], fmul2(L.x, wl[e]));
-                    const u64 uy = ffma2(R.y, wh[e], fmul2(L.y, wl[e]));
+                    u64 Lx, Ly, Rx, Ry;                // (z, Mx'), (My', Mxy') of the interval's two knots
+                    asm("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Lx), "=l"(Ly) : "r"(qc[e] + ro));
+                    asm("ld.shared.v2.b64 {%0, %1}, [%2+16];" : "=l"(Rx), "=l"(Ry) : "r"(qc[e] + ro));
+                    const u64 ux = ffma2(Rx, wh[e], fmul2(Lx, wl[e]));
+                    const u64 uy = ffma2(Ry, wh[e], fmul2(Ly, wl[e]));
                     xv[e] = lo_of(ux) + hi_of(ux);
                     yv[e] = lo_of(uy) + hi_of(uy);
                 }
@@ -337,61 +341,42 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
 #pragma unroll
             for (int p = 0; p < 2; ++p) X0[p] = X1[p] = Xd[p] = Y0[p] = Y1[p] = pack2(0.0f, 0.0f);
             const bool full = !oob_rows && (Jp + 128 <= Jend);        // warp-uniform
-            int curk = -2;
-            // (rolled: the unrolled form is several thousand instructions, more than the instruction cache
-            // holds for 16 warps at different places; lane i keeps rsv[i])
-            int rsv_lane = rsv[0];
-#pragma unroll
-            for (int i = 1; i <= TI; ++i) rsv_lane = (lane == i) ? rsv[i] : rsv_lane;
+            // Row-driven: the band's output rows in order; a row whose knot interval differs from the one
+            // before it (warp-uniform test) first moves the two knot rows on.  With up-sampling factor 2
+            // there are only two rows per interval, so nothing is set up per interval beyond that.
+            auto band = [&](auto full_c) {
+                constexpr bool FULL = decltype(full_c)::value;
+                int curj = -2;
+                const float4* rtp = rt_base;
+                float* op = out + (size_t)rb * ax.n_out + Jt;
 #pragma unroll 1
-            for (int ki = 0; ki < TI; ++ki) {
-                const int kj = kja + ki;
-                const int rs = __shfl_sync(0xffffffffu, rsv_lane, ki), re = __shfl_sync(0xffffffffu, rsv_lane, ki + 1);
-                if (kj >= kjb || rs >= re) continue;   // no such row of cells / no output row in it
-                if (kj == curk + 1) {
+                for (int r = rb; r < re; ++r, ++rtp, op += ax.n_out) {
+                    const float4 rc = *rtp;                               // (j, s, Cy, Dy); j < 0: outside the extent
+                    const int jr = __float_as_int(rc.x);
+                    const bool rv = FULL || jr >= 0;
+                    if (jr != curj && rv) {
+                        const int kj = jr - j0;
+                        if (jr != curj + 1) knot_row(kj, X1, Y1);         // first interval of the band only
 #pragma unroll
-                    for (int p = 0; p < 2; ++p) { X0[p] = X1[p]; Y0[p] = Y1[p]; }
-                } else {
-                    knot_row(kj, X0, Y0);
-                }
-                knot_row(kj + 1, X1, Y1);
+                        for (int p = 0; p < 2; ++p) { X0[p] = X1[p]; Y0[p] = Y1[p]; }
+                        knot_row(kj + 1, X1, Y1);
 #pragma unroll
-                for (int p = 0; p < 2; ++p) Xd[p] = ffma2(X0[p], neg1, X1[p]);
-                curk = kj;
-                float* op = out + (size_t)rs * ax.n_out + Jt;
-                if (full) {                            // all four columns inside the tile, no row outside the extent
-#pragma unroll 2
-                    for (int r = rs; r < re; ++r, op += ax.n_out) {
-                        const float4 rw = rt_ok ? s_rt[r - rt0] : __ldg(rowtab + r);   // (j, s, Cy, Dy)
-                        const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
-#pragma unroll
-                        for (int p = 0; p < 2; ++p) {
-                            u64 o = ffma2(s2, Xd[p], X0[p]);
-                            o = ffma2(cy2, Y0[p], o);
-                            o = ffma2(dy2, Y1[p], o);
-                            o = fadd2(o, zref2);
-                            op[64 * p] = lo_of(o);
-                            op[64 * p + 32] = hi_of(o);
-                        }
+                        for (int p = 0; p < 2; ++p) Xd[p] = ffma2(X0[p], neg1, X1[p]);
+                        curj = jr;
                     }
-                } else {
-#pragma unroll 1
-                    for (int r = rs; r < re; ++r, op += ax.n_out) {
-                        const float4 rw = rt_ok ? s_rt[r - rt0] : __ldg(rowtab + r);   // (j, s, Cy, Dy); j < 0: outside the extent
-                        const bool rv = __float_as_int(rw.x) >= 0;
-                        const u64 s2 = pack2(rw.y, rw.y), cy2 = pack2(rw.z, rw.z), dy2 = pack2(rw.w, rw.w);
+                    const u64 s2 = pack2(rc.y, rc.y), cy2 = pack2(rc.z, rc.z), dy2 = pack2(rc.w, rc.w);
 #pragma unroll
-                        for (int p = 0; p < 2; ++p) {
-                            u64 o = ffma2(s2, Xd[p], X0[p]);
-                            o = ffma2(cy2, Y0[p], o);
-                            o = ffma2(dy2, Y1[p], o);
-                            o = fadd2(o, zref2);
-                            if (cok[2 * p] && rv) op[64 * p] = lo_of(o);
-                            if (cok[2 * p + 1] && rv) op[64 * p + 32] = hi_of(o);
-                        }
+                    for (int p = 0; p < 2; ++p) {
+                        u64 o = ffma2(s2, Xd[p], X0[p]);
+                        o = ffma2(cy2, Y0[p], o);
+                        o = ffma2(dy2, Y1[p], o);
+                        o = fadd2(o, zref2);
+                        if (FULL || (cok[2 * p] && rv)) op[64 * p] = lo_of(o);
+                        if (FULL || (cok[2 * p + 1] && rv)) op[64 * p + 32] = hi_of(o);
                     }
                 }
-            }
+            };
+            if (full) band(std::true_type{}); else band(std::false_type{});
         }
     }
 }
