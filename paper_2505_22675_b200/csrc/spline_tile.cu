@@ -298,11 +298,12 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         // sweeps are dead): a global load per row would expose an L2 round trip in every interval
         constexpr int RT_CAP = (2 * NYI * PZ) / (4 * NW);                 // float4 entries per warp
         float4* s_rt = reinterpret_cast<float4*>(s_zf) + warp * RT_CAP;
-        const int rt_n = re - rb;
-        const bool rt_ok = rt_n <= RT_CAP;                               // warp-uniform
-        if (rt_ok) for (int i = lane; i < rt_n; i += 32) s_rt[i] = __ldg(rowtab + rb + i);
+        // (a band longer than the buffer -- up-sampling factors above ~40 -- goes through it in chunks)
+        for (int cb = rb; cb < re; cb += RT_CAP) {
+        const int ce = min(cb + RT_CAP, re);
         __syncwarp();
-        const float4* rt_base = rt_ok ? s_rt : rowtab + rb;              // row entry of output row rb
+        for (int i = lane; i < ce - cb; i += 32) s_rt[i] = __ldg(rowtab + cb + i);
+        __syncwarp();
         for (int Jp = Jbeg; Jp < Jend; Jp += 128) {
             const int Jt = Jp + lane;                  // column of e = 0; e-th column is 32 e further
             bool cok[4];
@@ -327,8 +328,8 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                     u64 Lx, Ly, Rx, Ry;                // (z, Mx'), (My', Mxy') of the interval's two knots
-                    asm("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Lx), "=l"(Ly) : "r"(qc[e] + ro));
-                    asm("ld.shared.v2.b64 {%0, %1}, [%2+16];" : "=l"(Rx), "=l"(Ry) : "r"(qc[e] + ro));
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Lx), "=l"(Ly) : "r"(qc[e] + ro) : "memory");
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2+16];" : "=l"(Rx), "=l"(Ry) : "r"(qc[e] + ro) : "memory");
                     const u64 ux = ffma2(Rx, wh[e], fmul2(Lx, wl[e]));
                     const u64 uy = ffma2(Ry, wh[e], fmul2(Ly, wl[e]));
                     xv[e] = lo_of(ux) + hi_of(ux);
@@ -347,11 +348,12 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
             auto band = [&](auto full_c) {
                 constexpr bool FULL = decltype(full_c)::value;
                 int curj = -2;
-                const float4* rtp = rt_base;
-                float* op = out + (size_t)rb * ax.n_out + Jt;
+                unsigned rtp = (unsigned)__cvta_generic_to_shared(s_rt);
+                float* op = out + (size_t)cb * ax.n_out + Jt;
 #pragma unroll 1
-                for (int r = rb; r < re; ++r, ++rtp, op += ax.n_out) {
-                    const float4 rc = *rtp;                               // (j, s, Cy, Dy); j < 0: outside the extent
+                for (int r = cb; r < ce; ++r, rtp += 16, op += ax.n_out) {
+                    float4 rc;                                            // (j, s, Cy, Dy); j < 0: outside the extent
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(rc.x), "=f"(rc.y), "=f"(rc.z), "=f"(rc.w) : "r"(rtp) : "memory");
                     const int jr = __float_as_int(rc.x);
                     const bool rv = FULL || jr >= 0;
                     if (jr != curj && rv) {
@@ -377,6 +379,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 }
             };
             if (full) band(std::true_type{}); else band(std::false_type{});
+        }
         }
     }
 }
