@@ -194,6 +194,22 @@ def test_spline_fused_worst_case_data(spline_path):
         assert max_abs_err(got, ref) <= TOL * depth_range(ref)
 
 
+@pytest.mark.parametrize("nx,ny,fy", [(100, 60, 60), (40, 40, 50), (120, 70, 45)])
+def test_spline_fused_long_bands(spline_path, nx, ny, fy):
+    # up-sampling factors in y so large that a warp's band of output rows is longer than its
+    # shared-memory row table (it is then walked in chunks)
+    rng = np.random.default_rng(79 + fy)
+    yy, xx = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    z = (-3000.0 + 20.0 * np.sin(xx / 3.0) * np.cos(yy / 4.0) + rng.normal(0, 1.0, (ny, nx))).astype(np.float32)
+    gi = W.Geom(nx, ny, 0.0, 0.0, 1.0, 1.0)
+    go = W.Geom(2 * nx + 3, (ny - 1) * fy + 7, -1.0, -3.0 / fy, 0.5, 1.0 / fy)     # a few nodes outside on each side
+    ref = _ref("spline", z, gi, go)
+    assert np.isnan(ref).any()
+    spline_path(1)
+    got = _run("spline", z, gi, go)
+    assert max_abs_err(got, ref) <= TOL * depth_range(ref)
+
+
 def test_spline_fused_path_refuses_what_it_cannot_serve(spline_path):
     b = _bathy()
     spline_path(1)
