@@ -350,10 +350,12 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 int curj = -2;
                 unsigned rtp = (unsigned)__cvta_generic_to_shared(s_rt);
                 float* op = out + (size_t)cb * ax.n_out + Jt;
-#pragma unroll 1
-                for (int r = cb; r < ce; ++r, rtp += 16, op += ax.n_out) {
+                auto lds_row = [&](unsigned addr) {
                     float4 rc;                                            // (j, s, Cy, Dy); j < 0: outside the extent
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(rc.x), "=f"(rc.y), "=f"(rc.z), "=f"(rc.w) : "r"(rtp) : "memory");
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(rc.x), "=f"(rc.y), "=f"(rc.z), "=f"(rc.w) : "r"(addr) : "memory");
+                    return rc;
+                };
+                auto one_row = [&](const float4 rc) {
                     const int jr = __float_as_int(rc.x);
                     const bool rv = FULL || jr >= 0;
                     if (jr != curj && rv) {
@@ -376,7 +378,17 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                         if (FULL || (cok[2 * p] && rv)) op[64 * p] = lo_of(o);
                         if (FULL || (cok[2 * p + 1] && rv)) op[64 * p + 32] = hi_of(o);
                     }
+                    op += ax.n_out;
+                };
+                // two rows per trip, both row entries in flight before the first is used
+                int r = cb;
+#pragma unroll 1
+                for (; r + 1 < ce; r += 2, rtp += 32) {
+                    const float4 ra = lds_row(rtp), rb2 = lds_row(rtp + 16);
+                    one_row(ra);
+                    one_row(rb2);
                 }
+                if (r < ce) one_row(lds_row(rtp));
             };
             if (full) band(std::true_type{}); else band(std::false_type{});
         }
