@@ -92,14 +92,24 @@ __device__ __forceinline__ void thomas_window(Rd rd, St st, int k0_rt, int nk_rt
     e[N - 2] = fmaf(-cp141(N - 4), e[N - 3], fmaf(-1.0f / 6.0f, e[N - 1], e[N - 2]));
 #pragma unroll
     for (int q = N - 3; q >= 1; --q) e[q] = fmaf(-cp141(q), e[q + 1], e[q]);   // pass 3: backward sweep, wt_q in place
-    // pass 4: M'_q = z_q - 6 c'_q wt_q on the kept knots (the knot is read again: no second register array)
+    // pass 4: M'_q = z_q - 6 c'_q wt_q on the kept knots (the knot is read again: no second register
+    // array).  Reads and writes go in groups of 8: the compiler cannot prove that the stores do not
+    // alias the knots, so a store between two loads would serialise them (one shared-memory latency
+    // per knot: this was 20 % of the kernel's warp time).
     if (N - 1 - k0 >= 0 && N - 1 - k0 < nk) st(N - 1 - k0, rd(N - 1), 0.0f);
+    constexpr int B = 8;
 #pragma unroll
-    for (int q = N - 2; q >= 1; --q) {
-        const int k = q - k0;
-        if (k >= 0 && k < nk) {
-            const float v = rd(q);
-            st(k, v, fmaf(-6.0f * cp141(q - 1), e[q], v));
+    for (int qb = N - 2; qb >= 1; qb -= B) {
+        float v[B];
+#pragma unroll
+        for (int g = 0; g < B; ++g) {
+            const int q = qb - g, k = q - k0;
+            v[g] = (q >= 1 && k >= 0 && k < nk) ? rd(q) : 0.0f;
+        }
+#pragma unroll
+        for (int g = 0; g < B; ++g) {
+            const int q = qb - g, k = q - k0;
+            if (q >= 1 && k >= 0 && k < nk) st(k, v[g], fmaf(-6.0f * cp141(q >= 1 ? q - 1 : 0), e[q >= 1 ? q : 0], v[g]));
         }
     }
     if (k0 == 0) st(0, rd(0), 0.0f);
