@@ -237,8 +237,6 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const int Ibeg = __ldg(tby + byt), Iend = __ldg(tby + byt + 1);
         const int offx = w0x & 3;
         const float* s_z = s_zbuf;
-        float zref = __ldg(in + (size_t)w0y * ax.n_in + w0x);
-        if (!isfinite(zref)) zref = 0.0f;
         // the warp's band: knot intervals [kja, kjb) of the tile = output rows [rb, re) (rfirst[j]: first
         // output row whose interval is >= j)
         constexpr int TI = (TYI + NW - 1) / NW;                           // knot intervals per warp
@@ -247,6 +245,18 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const int re = (kjb > kja) ? min(max(__ldg(rfirst + min(j0 + kjb, ay.n_in)), Ibeg), Iend) : rb;
         asm volatile("cp.async.wait_group 0;" ::: "memory");             // the window has landed
         __syncthreads();
+        float zref = s_z[offx];                                           // the window's first sample
+        if (!isfinite(zref)) zref = 0.0f;
+        // the table entries the evaluate stage starts with: into L1 now, two stages ahead of their use
+        for (int i = rb + lane; i < re; i += 32) asm volatile("prefetch.global.L1 [%0];" :: "l"(rowtab + i));
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int J = Jbeg + lane + 32 * e;
+            if (J < Jend) {
+                asm volatile("prefetch.global.L1 [%0];" :: "l"(colw + J));
+                asm volatile("prefetch.global.L1 [%0];" :: "l"(coli + J));
+            }
+        }
 
         // ---- S2: Thomas along y of every window column (one thread per column): z - zref and My' on the
         //      tile's knot rows, into odd-pitch planes that the row-wise solves read without bank conflicts
