@@ -168,6 +168,21 @@ BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, i
                grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
                void* cuda_stream);
 
+/* The same three, ENQUEUED only: scratch allocation, copies, kernels and releases are all ordered on
+ * `cuda_stream` and the call returns without waiting for them (krige_host_async waits once, on its
+ * own stream, for the soundings' bounding box -- see krige_build_index).  The host buffers must be
+ * pinned (otherwise the copies fall back to synchronous staging) and must stay valid, and h_out /
+ * h_zhat / *h_failed_or_null are defined, only after the caller has synchronised `cuda_stream`.
+ * Issued on different streams, the copies of one call overlap the kernels and the opposite-direction
+ * copies of another: the way to run the three methods of a survey step at PCIe speed
+ * (bench.py's `e2e`).  Errors detected at enqueue time are returned; later ones surface at the
+ * caller's synchronisation. */
+BATHY_API int interp_bilinear_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
+BATHY_API int interp_spline_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
+BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
+               grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
+               void* cuda_stream);
+
 /* Selects the implementation interp_spline uses (process-wide; for tests and profiling):
  * 0 = automatic (default): the fused single-pass tile kernel where it applies (up-sampling, input at
  *     least one solve window wide), else the global-solve path;

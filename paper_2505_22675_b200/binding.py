@@ -23,7 +23,8 @@ MAX_K = 64
 
 SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
            "krige_predict", "krige_free_index", "krige_free_index_async", "krige_index_info", "interp_bilinear_host",
-           "interp_spline_host", "krige_host", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path"]
+           "interp_spline_host", "krige_host", "interp_bilinear_host_async", "interp_spline_host_async",
+           "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path"]
 
 
 class GridGeom(C.Structure):
@@ -69,6 +70,9 @@ def lib():
         L.interp_bilinear_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
         L.interp_spline_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
         L.krige_host.argtypes = [vp, vp, vp, C.c_int64, C.c_float, GridGeom, Variogram, C.c_int32, vp, vp, vp]
+        L.interp_bilinear_host_async.argtypes = L.interp_bilinear_host.argtypes
+        L.interp_spline_host_async.argtypes = L.interp_spline_host.argtypes
+        L.krige_host_async.argtypes = L.krige_host.argtypes
         L.bathy_strerror.argtypes = [C.c_int]
         L.bathy_strerror.restype = C.c_char_p
         L.bathy_launch_count.restype = C.c_int64
@@ -247,6 +251,38 @@ def interp_spline_host(z, gin, gout, out=None, stream=None):
     out, op = _host_f32(out, "out")
     _check(lib().interp_spline_host(zp, gi, op, go, _stream(stream)), "interp_spline_host")
     return out
+
+
+def _pinned_f32(a, name):
+    if not isinstance(a, torch.Tensor) or a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous() or not a.is_pinned():
+        raise TypeError(f"{name} must be a contiguous pinned float32 host tensor (torch.Tensor.pin_memory())")
+    return a.data_ptr()
+
+
+def interp_bilinear_host_async(z, gin, gout, out, stream=None):
+    """Enqueue only (include/bathy.h): `out` is defined after the caller synchronises `stream`."""
+    _check(lib().interp_bilinear_host_async(_pinned_f32(z, "z"), _geom(gin), _pinned_f32(out, "out"), _geom(gout),
+                                            _stream(stream)), "interp_bilinear_host_async")
+    return out
+
+
+def interp_spline_host_async(z, gin, gout, out, stream=None):
+    """Enqueue only (include/bathy.h): `out` is defined after the caller synchronises `stream`."""
+    _check(lib().interp_spline_host_async(_pinned_f32(z, "z"), _geom(gin), _pinned_f32(out, "out"), _geom(gout),
+                                          _stream(stream)), "interp_spline_host_async")
+    return out
+
+
+def krige_host_async(x, y, z, gout, model, range_, sill, nugget, k, out, failed, cell_size: float = 0.0, stream=None):
+    """Enqueue only (include/bathy.h): `out` and `failed` (a pinned int64 tensor of one element) are
+    defined after the caller synchronises `stream`."""
+    if not isinstance(failed, torch.Tensor) or failed.dtype != torch.int64 or failed.numel() != 1 or not failed.is_pinned():
+        raise TypeError("failed must be a pinned int64 host tensor of one element")
+    vg = Variogram(int(model), float(range_), float(sill), float(nugget))
+    _check(lib().krige_host_async(_pinned_f32(x, "x"), _pinned_f32(y, "y"), _pinned_f32(z, "z"), x.numel(), float(cell_size),
+                                  _geom(gout), vg, int(k), _pinned_f32(out, "out"), failed.data_ptr(), _stream(stream)),
+           "krige_host_async")
+    return out, failed
 
 
 def krige_host(x, y, z, gout, model, range_, sill, nugget, k, cell_size: float = 0.0, out=None, stream=None):

@@ -118,7 +118,13 @@ BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell
     return BATHY_OK;
 }
 
-BATHY_API int interp_bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+}  // extern "C"
+
+namespace {
+
+// The host-buffer forms: `wait` = synchronise the stream before returning (the plain forms), else
+// everything (allocations, copies, kernels, releases) is only enqueued on the stream (`*_async`).
+int bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream, bool wait)
 {
     if (!h_in || !h_out) return BATHY_ERR_NULL;
     int rc = check_in_geom(in);
@@ -133,11 +139,11 @@ BATHY_API int interp_bilinear_host(const float* h_in, grid_geom_t in, float* h_o
     rc = launch_bilinear(static_cast<const float*>(din.p), in, static_cast<float*>(dout.p), out, s);
     if (rc) return rc;
     BATHY_CUDA_TRY(cudaMemcpyAsync(h_out, dout.p, nout, cudaMemcpyDeviceToHost, s));
-    BATHY_CUDA_TRY(cudaStreamSynchronize(s));
+    if (wait) BATHY_CUDA_TRY(cudaStreamSynchronize(s));
     return BATHY_OK;
 }
 
-BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+int spline_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream, bool wait)
 {
     if (!h_in || !h_out) return BATHY_ERR_NULL;
     int rc = check_in_geom(in);
@@ -152,13 +158,13 @@ BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out
     rc = launch_spline(static_cast<const float*>(din.p), in, static_cast<float*>(dout.p), out, ws.p, s, g_spline_path.load());
     if (rc) return rc;
     BATHY_CUDA_TRY(cudaMemcpyAsync(h_out, dout.p, nout, cudaMemcpyDeviceToHost, s));
-    BATHY_CUDA_TRY(cudaStreamSynchronize(s));
+    if (wait) BATHY_CUDA_TRY(cudaStreamSynchronize(s));
     return BATHY_OK;
 }
 
-BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
-               grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
-               void* cuda_stream)
+int krige_host_impl(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
+                    grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
+                    void* cuda_stream, bool wait)
 {
     if (!h_x || !h_y || !h_z || !h_zhat) return BATHY_ERR_NULL;
     if (n < 1 || n > 0x7fffffffLL) return BATHY_ERR_SIZE;
@@ -185,12 +191,33 @@ BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, i
         cudaError_t e = cudaMemcpyAsync(h_zhat, dout.p, nout, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess && h_failed_or_null)
             e = cudaMemcpyAsync(h_failed_or_null, dfail.p, sizeof(int64_t), cudaMemcpyDeviceToHost, s);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e == cudaSuccess && wait) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) rc = BATHY_ERR_CUDA;
     }
-    free_index(idx);
+    free_index_async(idx, s);
     return rc;
 }
+
+}  // namespace
+
+extern "C" {
+
+BATHY_API int interp_bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+{ return bilinear_host(h_in, in, h_out, out, cuda_stream, true); }
+BATHY_API int interp_bilinear_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+{ return bilinear_host(h_in, in, h_out, out, cuda_stream, false); }
+BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+{ return spline_host(h_in, in, h_out, out, cuda_stream, true); }
+BATHY_API int interp_spline_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+{ return spline_host(h_in, in, h_out, out, cuda_stream, false); }
+BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
+               grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
+               void* cuda_stream)
+{ return krige_host_impl(h_x, h_y, h_z, n, cell_size, out, vg, k, h_zhat, h_failed_or_null, cuda_stream, true); }
+BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
+               grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
+               void* cuda_stream)
+{ return krige_host_impl(h_x, h_y, h_z, n, cell_size, out, vg, k, h_zhat, h_failed_or_null, cuda_stream, false); }
 
 BATHY_API const char* bathy_strerror(int status)
 {

@@ -242,3 +242,33 @@ def test_stream_ordered_release_and_rebuild():
     for o in outs[1:]:
         assert torch.equal(o, outs[0])
     assert torch.isfinite(outs[0]).all()
+
+
+def test_async_host_forms_on_three_streams():
+    # the enqueue-only host forms (include/bathy.h): three methods on three streams, results
+    # defined after the streams are synchronised, bit-identical to the device-pointer forms
+    b = _bathy()
+    w = W.sounding_config(4, width=150.0, n_target=5600, n_out=96)
+    gw = W.grid_config(2, n_in=129, factor=4, n_features=10)
+    dev_k, _, _, _ = _gpu(w.x, w.y, w.z, w.geom_out, w.model, w.range_, w.sill, w.nugget, w.k, want_nbr=False)
+    zt = torch.from_numpy(gw.z).cuda()
+    dev_b = b.interp_bilinear(zt, gw.geom_in, gw.geom_out).cpu().numpy()
+    dev_s = b.interp_spline(zt, gw.geom_in, gw.geom_out).cpu().numpy()
+    hx, hy, hz = (torch.from_numpy(a).pin_memory() for a in (w.x, w.y, w.z))
+    hg = torch.from_numpy(gw.z).pin_memory()
+    ok = torch.full(w.geom_out.shape, -1.0, dtype=torch.float32).pin_memory()
+    ob = torch.full(gw.geom_out.shape, -1.0, dtype=torch.float32).pin_memory()
+    os_ = torch.full(gw.geom_out.shape, -1.0, dtype=torch.float32).pin_memory()
+    failed = torch.full((1,), -1, dtype=torch.int64).pin_memory()
+    sk, sb, ss = (torch.cuda.Stream() for _ in range(3))
+    for _ in range(3):                                   # repeated: scratch comes from and returns to the stream pool
+        b.krige_host_async(hx, hy, hz, w.geom_out, w.model, w.range_, w.sill, w.nugget, w.k, out=ok, failed=failed, stream=sk)
+        b.interp_bilinear_host_async(hg, gw.geom_in, gw.geom_out, out=ob, stream=sb)
+        b.interp_spline_host_async(hg, gw.geom_in, gw.geom_out, out=os_, stream=ss)
+        for s_ in (sk, sb, ss):
+            s_.synchronize()
+        assert int(failed[0]) == 0
+        assert np.array_equal(ok.numpy(), dev_k) and np.array_equal(ob.numpy(), dev_b) and np.array_equal(os_.numpy(), dev_s)
+        ok.fill_(-1.0); ob.fill_(-1.0); os_.fill_(-1.0)
+    with pytest.raises(TypeError):
+        b.interp_bilinear_host_async(torch.from_numpy(gw.z), gw.geom_in, gw.geom_out, out=ob)      # not pinned
