@@ -52,7 +52,9 @@ struct TileShape {
                                                        // 0..3 columns between the aligned start and the window start
     static constexpr int PQ = NXI;                     // pitch of the knot records Q = (z, Mx', My', Mxy'), in float4
     static constexpr int front_floats = (4 * NYI * PQ > WY * PA) ? 4 * NYI * PQ : WY * PA;   // max(knot records, raw window)
-    static constexpr size_t smem_bytes = sizeof(float) * ((size_t)front_floats + 2 * (size_t)NYI * PZ);
+    static constexpr int PSK = (16 - (NYI * PZ) % 32 + 32) % 32;   // skew of the second plane: the two planes of a
+                                                       // knot row sit 16 banks apart (x sweeps, below)
+    static constexpr size_t smem_bytes = sizeof(float) * ((size_t)front_floats + 2 * (size_t)NYI * PZ + PSK);
     static_assert(WX <= kTileThreads && 2 * NYI <= kTileThreads && NYI <= 32, "tile shape");
 };
 
@@ -170,7 +172,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
     float4* s_q = reinterpret_cast<float4*>(s_raw);                       // [NYI][PQ] knot records (z, Mx', My', Mxy')
     float* s_zbuf = reinterpret_cast<float*>(s_raw);                      // [WY][PA] raw window
     float* s_zf = reinterpret_cast<float*>(s_raw) + S::front_floats;      // [NYI][PZ] z - zref on the tile's knot rows
-    float* s_my = s_zf + NYI * PZ;                                        // [NYI][PZ] My' on the tile's knot rows
+    float* s_my = s_zf + NYI * PZ + S::PSK;                               // [NYI][PZ] My' on the tile's knot rows
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const bool vec_ok = (reinterpret_cast<uintptr_t>(in) & 15) == 0 && (ax.n_in & 3) == 0;
@@ -273,16 +275,22 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         // ---- S1: Mx' = Thomas along x of z on the knot rows (warp 0 -> Q.xy = (z, Mx'));
         //      S3: Mxy' = Thomas along x of My' (warp 1 -> Q.zw = (My', Mxy'))
         if (inner_x) {
-            // interior tile: every warp works -- plane = warp & 1 (z or My'), half = warp >> 1: the row's
+            // interior tile: every warp works; the row's
             // knots are solved as two overlapping windows of HW = TXI/2 + 1 + 2H knots (the same
             // 0.268^H bound applies where the halves meet), so the serial chains are 55 instead of 87 long
             constexpr int HL = TXI / 2 + 1;                               // knots kept by the left half
             constexpr int HW = HL + 2 * H;                                // window of a half
-            if (lane < nky) {
-                const int plane = warp & 1, half = warp >> 1;
-                const float* row = (plane == 0 ? s_zf : s_my) + lane * PZ + (half ? WX - HW : 0);
+            // A warp takes one half and 16 knot rows, both planes: lanes 0-7 / 8-15 are plane 0 / 1 of
+            // rows 0-7, lanes 16-31 the same of rows 8-15.  A half-warp then writes 8 records' (z, Mx')
+            // and (My', Mxy') halves = 16 different 8-byte bank pairs: the STS.64 are conflict-free
+            // (a warp of one plane writes 4-way conflicting: this was a tenth of the kernel's
+            // shared-memory wavefronts, the unit that bounds it), and so are the loads (plane skew PSK).
+            const int plane = (lane >> 3) & 1, half = warp >> 1;
+            const int krow = 16 * (warp & 1) + (lane & 7) + 8 * (lane >> 4);
+            if (krow < nky) {
+                const float* row = (plane == 0 ? s_zf : s_my) + krow * PZ + (half ? WX - HW : 0);
                 static_assert(WX - HW == HL - 1 && NXI - HL == HL - 1, "the halves share one instantiation");
-                float2* dst = reinterpret_cast<float2*>(s_q + lane * PQ + (half ? HL - 1 : 0)) + plane;
+                float2* dst = reinterpret_cast<float2*>(s_q + krow * PQ + (half ? HL - 1 : 0)) + plane;
                 auto rd = [&](int q) { return row[q]; };
                 // left: window knots [0, HW), kept = tile knots [0, HL) = window [H, H + HL)
                 // right: window knots [WX - HW, WX), window [H, H + HL) = tile knots [HL - 1, NXI): the same
