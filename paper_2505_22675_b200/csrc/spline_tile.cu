@@ -88,16 +88,33 @@ __device__ __forceinline__ void thomas_window(Rd rd, St st, int k0_rt, int nk_rt
     float e[N];
 #pragma unroll
     for (int q = 0; q < N; ++q) e[q] = rd(q);                          // pass 1: the knots
+    // interior tiles keep the knots they will write out in registers (a second read of shared memory
+    // costs wavefronts of the unit that bounds the kernel); edge tiles read them again in pass 4
+    constexpr int NV = STATIC ? NK : 1;
+    float vk[NV];
+    if (STATIC) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) vk[k] = e[K0 + k];
+    }
     e[1] = fmaf(-1.0f / 6.0f, e[0], e[1]);                             // pass 2: forward sweep, e_q in place
 #pragma unroll
     for (int q = 2; q <= N - 3; ++q) e[q] = fmaf(-cp141(q - 2), e[q - 1], e[q]);
     e[N - 2] = fmaf(-cp141(N - 4), e[N - 3], fmaf(-1.0f / 6.0f, e[N - 1], e[N - 2]));
 #pragma unroll
     for (int q = N - 3; q >= 1; --q) e[q] = fmaf(-cp141(q), e[q + 1], e[q]);   // pass 3: backward sweep, wt_q in place
-    // pass 4: M'_q = z_q - 6 c'_q wt_q on the kept knots (the knot is read again: no second register
-    // array).  Reads and writes go in groups of 8: the compiler cannot prove that the stores do not
-    // alias the knots, so a store between two loads would serialise them (one shared-memory latency
-    // per knot: this was 20 % of the kernel's warp time).
+    // pass 4: M'_q = z_q - 6 c'_q wt_q on the kept knots.  Where the knot is read again, reads and writes
+    // go in groups of 8: the compiler cannot prove that the stores do not alias the knots, so a store
+    // between two loads would serialise them (one shared-memory latency per knot: this was 20 % of the
+    // kernel's warp time).
+    if (STATIC) {
+        static_assert(!STATIC || (K0 >= 1 && K0 + NK <= N - 1), "kept knots are interior knots of the window");
+#pragma unroll
+        for (int k = NV - 1; k >= 0; --k) {
+            const int q = K0 + k;
+            st(k, vk[k], fmaf(-6.0f * cp141(q - 1), e[q], vk[k]));
+        }
+        return;
+    }
     if (N - 1 - k0 >= 0 && N - 1 - k0 < nk) st(N - 1 - k0, rd(N - 1), 0.0f);
     constexpr int B = 8;
 #pragma unroll
