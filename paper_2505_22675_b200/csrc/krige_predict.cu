@@ -68,7 +68,11 @@ struct Shape {
     static constexpr int WARPS = (K <= 32) ? 16 : 8;           // warps per CTA: one CTA per SM (registers)
     static constexpr int NQ = CAP / 32;
     static constexpr int XYS = K + 4;           // float stride of a node's coordinate lists (bank skew)
-    static constexpr int CBS = K + 4;           // float stride of a node's column buffer (bank skew)
+    // float stride of a node's column buffer: = G (mod 32), so that the NB x G lanes of a warp, each
+    // storing one entry of its node's column, hit 32 different banks (K + 4 gave 2-way conflicts)
+    static constexpr int CBS = K + ((G - K) % 32 + 32) % 32;
+    static constexpr int NBLP = 33;             // pitch of the per-lane uint16 lists: 16.5 words, so that one lane's
+                                                // column (the gather before the solve) spreads over all banks
 };
 
 template <int K, int G>
@@ -84,7 +88,7 @@ struct __align__(16) WarpSmem {
     float    cz[S::CAP];                        //             depth (pilot: key bits)
     int32_t  cid[S::CAP];                       //             original index
     uint16_t hist[kBuckets + 1][32];            // per-lane key histogram (column = lane)
-    uint16_t nbl[K][32];                        // per-lane neighbour list: candidate slots
+    uint16_t nbl[K][S::NBLP];                   // per-lane neighbour list: candidate slots
     uint16_t crit[kCrit][32];                   // per-lane candidates of the critical bucket
 };
 
