@@ -71,6 +71,7 @@ struct Shape {
     // float stride of a node's column buffer: = G (mod 32), so that the NB x G lanes of a warp, each
     // storing one entry of its node's column, hit 32 different banks (K + 4 gave 2-way conflicts)
     static constexpr int CBS = K + ((G - K) % 32 + 32) % 32;
+    static constexpr bool ILV = (K > 32);       // lane <-> (node, row group) mapping of the solve, see solve_batch
     static constexpr int NBLP = 33;             // pitch of the per-lane uint16 lists: 16.5 words, so that one lane's
                                                 // column (the gather before the solve) spreads over all banks
 };
@@ -361,6 +362,10 @@ __device__ __forceinline__ u64 cov2_scaled(u64 h2, const PredictParams& p)
 
 // K3-K5 for the NB nodes whose neighbour lists (scaled coordinates relative to the block centre,
 // depths) sit in ws.nb_x, ws.nb_y, ws.nb_z.  Lane (nd, g) = (lane / G, lane % G) holds rows g, g+G, ...
+// (at k = 64 the nodes are interleaved instead, (nd, g) = (lane % NB, lane / NB): the NB owners of a row
+// are then neighbouring lanes and their 16-byte stores of the published row one shared-memory wavefront
+// -- a 128-bit store is split by quarter-warp.  Measured: k = 64 6.66 -> 6.40 ms per 1 M nodes; at k = 32
+// the broadcast column loads get slower by more than the stores gain, 5.55 -> 6.02 ms)
 // of node nd, two columns to a 64-bit register pair.  Rows at or beyond k are pad soundings placed
 // far away from everything (covariance exactly 0): they decouple as identity rows with zero
 // right-hand sides.
@@ -371,7 +376,7 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
     using S = Shape<K, G>;
     constexpr int R = S::R;
     static_assert(G % 2 == 0 && K % 4 == 0, "column pairs must not straddle a row block");
-    const int nd = lane / G, g = lane % G;
+    const int nd = S::ILV ? lane % S::NB : lane / G, g = S::ILV ? lane / S::NB : lane % G;
     const int k = p.k;
     const float zref = ws.nb_z[nd][0];
 
@@ -603,7 +608,7 @@ krige_predict_kernel(const PredictParams p)
                     ws.nb_z[nd][m] = z;
                 }
                 __syncwarp();
-                const int src = bb * S::NB + lane / G;     // the lane whose node this lane helps to solve
+                const int src = bb * S::NB + (S::ILV ? lane % S::NB : lane / G);   // the lane whose node this lane helps to solve
                 const int Js = bj * BW + (src & (BW - 1)), Is = bi * BH + (src / BW);
                 // __fmul_rn: no contraction into the subtractions of the solve, so that a node on a
                 // datum sees h2 == 0 exactly (same expression as the neighbour's coordinates)
