@@ -452,10 +452,13 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
             const int t1 = (j + 1) / G, g1 = (j + 1) % G;
             const float a1 = ((j + 1) & 1) ? hi_of(A2[t1][(j + 1) / 2]) : lo_of(A2[t1][(j + 1) / 2]);
             const float pv = fmaf(nLr[t1], -nLr[t1], a1);
-            if (g == g1) ws.rhs[buf][nd] = make_float4(lo_of(yz1[t1]), hi_of(yz1[t1]), yc[t1], pv);
+            // from the row's owner to the lanes of its node: four shuffles (a 16-byte store by the 4
+            // owners, one per quarter-warp, plus the load back cost 6 shared-memory wavefronts)
+            const int owner = S::ILV ? (lane % S::NB) + S::NB * g1 : (lane & ~(G - 1)) | g1;
+            P.x = __shfl_sync(kFull, yz1[t1], owner);
+            P.y = pack2(__shfl_sync(kFull, yc[t1], owner), __shfl_sync(kFull, pv, owner));
         }
         __syncwarp();
-        if (j + 1 < K) P = *reinterpret_cast<const ulonglong2*>(&ws.rhs[buf][nd]);
 #pragma unroll
         for (int m4 = (j + 1) / 4; m4 < K / 4; ++m4) {
             const ulonglong2 L4 = *reinterpret_cast<const ulonglong2*>(&ws.colbuf[buf][nd][4 * m4]);
