@@ -79,7 +79,7 @@ struct Shape {
 template <int K, int G>
 struct __align__(16) WarpSmem {
     using S = Shape<K, G>;
-    float4   rhs[2][S::NB];                     // -(y_c, y_1, y_z) of the current column, per node
+    float4   rhs[2][S::NB];                     // (rhs_z, rhs_1, rhs_c, pivot) of row 0, per node (slot [1])
     float    colbuf[2][S::NB][S::CBS];          // -(column j of L), per node (double buffered)
     float    nb_x[S::NB][S::XYS];               // neighbour coordinates, scaled, relative to the block centre
     float    nb_y[S::NB][S::XYS];
@@ -362,10 +362,8 @@ __device__ __forceinline__ u64 cov2_scaled(u64 h2, const PredictParams& p)
 
 // K3-K5 for the NB nodes whose neighbour lists (scaled coordinates relative to the block centre,
 // depths) sit in ws.nb_x, ws.nb_y, ws.nb_z.  Lane (nd, g) = (lane / G, lane % G) holds rows g, g+G, ...
-// (at k = 64 the nodes are interleaved instead, (nd, g) = (lane % NB, lane / NB): the NB owners of a row
-// are then neighbouring lanes and their 16-byte stores of the published row one shared-memory wavefront
-// -- a 128-bit store is split by quarter-warp.  Measured: k = 64 6.66 -> 6.40 ms per 1 M nodes; at k = 32
-// the broadcast column loads get slower by more than the stores gain, 5.55 -> 6.02 ms)
+// (at k = 64 the nodes are interleaved instead, (nd, g) = (lane % NB, lane / NB).  Measured: k = 64 6.07 ->
+// 5.98 ms per 1 M nodes; at k = 32 the broadcast column loads get slower, 5.55 -> 6.02 ms)
 // of node nd, two columns to a 64-bit register pair.  Rows at or beyond k are pad soundings placed
 // far away from everything (covariance exactly 0): they decouple as identity rows with zero
 // right-hand sides.
@@ -416,10 +414,12 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
 
     // K4: right-looking Cholesky, column by column; the three right-hand sides are forward-substituted
     // on the way and their four dot products (the Schur step, K5) accumulate as the y_j appear.
-    // Row j's owner publishes P_j = (rhs_z, rhs_1, rhs_c, pivot) of its row -- final once column j-1
-    // has been applied, which it can do for its own row before anybody else has seen that column --
-    // in the same phase as column j-1 itself: one __syncwarp per column, no shuffles, and the rsqrt
-    // of the next pivot overlaps the trailing update.
+    // Row j's owner hands P_j = (rhs_z, rhs_1, rhs_c, pivot) of its row to the lanes of its node -- final
+    // once column j-1 has been applied, which it can do for its own row before anybody else has seen
+    // that column -- in the same phase as column j-1 itself, by four shuffles: one __syncwarp per
+    // column, and the rsqrt of the next pivot overlaps the trailing update.  (Row 0 goes through
+    // ws.rhs once: replacing that by shuffles too changes nothing at k = 32 and costs 2 % at k = 64,
+    // where the kernel is at the register limit.)
     float pmin = 1.0f;               // smallest pivot (a NaN pivot poisons every later column and the estimate)
     u64 dots_c = pack2(0.0f, 0.0f);  // (y_c.y_z, y_c.y_1)
     u64 dots_1 = pack2(0.0f, 0.0f);  // (y_1.y_z, y_1.y_1)
