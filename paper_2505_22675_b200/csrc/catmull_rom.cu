@@ -90,8 +90,8 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     bool cok[CPT], c4ok[CPT];                         // column inside the tile / has its 4 x neighbours in the grid
     float ct[CPT], cnan[CPT];
     float cw0[CPT], cw2[CPT], cw3[CPT];               // x weights of P0, P2, P3 (P1's is 1 minus their sum)
-    int c1[CPT], cl[CPT], cr[CPT];                    // offset of P1 in a footprint row; P0 at c1 - cl, P3 at c1 + 1 + cr
-                                                      // (cl, cr in {0, 1}: clamped into the footprint)
+    unsigned o1[CPT], o0[CPT], o3[CPT];               // byte offsets of P1, P0, P3 in a footprint row (P2 at o1 + 4; P0 and
+                                                      // P3 clamped into the footprint): a shared-memory address is one add
     const float qnan = __int_as_float(0x7fc00000);
 #pragma unroll
     for (int e = 0; e < CPT; ++e) {
@@ -104,10 +104,14 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         c4ok[e] = (i >= 1) && (i + 2 <= ax.n_in - 1);
         const float4 w = cr_weights(ct[e]);
         cw0[e] = w.x; cw2[e] = w.z; cw3[e] = w.w;
-        c1[e] = min(max(ic, fi0), fi1 - 1) - fi0 + offx;
-        cl[e] = (c1[e] - 1 >= offx) ? 1 : 0;
-        cr[e] = (c1[e] + 2 <= fi1 - fi0 + offx) ? 1 : 0;
+        const int c1 = min(max(ic, fi0), fi1 - 1) - fi0 + offx;
+        o1[e] = 4u * (unsigned)c1;
+        o0[e] = (c1 - 1 >= offx) ? o1[e] - 4u : o1[e];
+        o3[e] = (c1 + 2 <= fi1 - fi0 + offx) ? o1[e] + 8u : o1[e] + 4u;
     }
+    const unsigned tile_sa = (unsigned)__cvta_generic_to_shared(s_tile);
+    auto lds = [](unsigned a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); return v; };
+    auto lds4 = [](unsigned a) { float v; asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(a) : "memory"); return v; };
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
 
@@ -131,16 +135,15 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
             X2[0] = X2[1] = pack2(qnan, qnan);
             return true;
         }
-        const float* row = s_tile + (jrow - fj0) * pitch;
+        const unsigned row = tile_sa + 4u * (unsigned)((jrow - fj0) * pitch);
 #pragma unroll
         for (int p = 0; p < CPT / 2; ++p) {
-            const float* qa = row + c1[2 * p];
-            const float* qb = row + c1[2 * p + 1];
-            const u64 p1 = pack2(qa[0], qb[0]);
+            const unsigned qa = row + o1[2 * p], qb = row + o1[2 * p + 1];
+            const u64 p1 = pack2(lds(qa), lds(qb));
             const u64 np1 = fmul2(p1, neg1);
-            const u64 d0 = fadd2(pack2(qa[-cl[2 * p]], qb[-cl[2 * p + 1]]), np1);
-            const u64 d2 = fadd2(pack2(qa[1], qb[1]), np1);
-            const u64 d3 = fadd2(pack2(qa[1 + cr[2 * p]], qb[1 + cr[2 * p + 1]]), np1);
+            const u64 d0 = fadd2(pack2(lds(row + o0[2 * p]), lds(row + o0[2 * p + 1])), np1);
+            const u64 d2 = fadd2(pack2(lds4(qa), lds4(qb)), np1);
+            const u64 d3 = fadd2(pack2(lds(row + o3[2 * p]), lds(row + o3[2 * p + 1])), np1);
             X2[p] = ffma2(w3x[p], d3, ffma2(w2x[p], d2, ffma2(w0x[p], d0, fadd2(p1, nzr[p]))));
         }
         const u64 t = fadd2(X2[0], X2[1]);
@@ -149,11 +152,11 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     };
     // x lerp of input row jrow (always inside the grid) for the bilinear fallback
     auto row_lerp = [&](int jrow, float* L) {
-        const float* row = s_tile + (jrow - fj0) * pitch;
+        const unsigned row = tile_sa + 4u * (unsigned)((jrow - fj0) * pitch);
 #pragma unroll
         for (int e = 0; e < CPT; ++e) {
-            const float p1 = row[c1[e]];
-            L[e] = fmaf(ct[e], row[c1[e] + 1] - p1, p1 - zref);
+            const float p1 = lds(row + o1[e]);
+            L[e] = fmaf(ct[e], lds4(row + o1[e]) - p1, p1 - zref);
         }
     };
 
