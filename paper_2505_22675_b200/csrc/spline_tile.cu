@@ -145,6 +145,9 @@ spline_tables_kernel(AxisMap ax, AxisMap ay, float4* __restrict__ colw, float4* 
                      int* __restrict__ tbx, int* __restrict__ tby, int* __restrict__ rfirst, int* __restrict__ coli,
                      int nbx, int nby, int txi, int tyi)
 {
+    // the tile kernel is launched with programmatic stream serialisation: its CTAs may start (and load
+    // their windows) while this grid still runs; they wait (griddepcontrol.wait) before reading a table
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     int n = blockIdx.x * 256 + threadIdx.x;
     if (n < ax.n_out + ay.n_out) {
         const bool isx = n < ax.n_out;
@@ -252,6 +255,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
                 }
             }
         }
+        asm volatile("griddepcontrol.wait;" ::: "memory");               // the tables of this call are complete
         const int Jbeg = __ldg(tbx + bxt), Jend = __ldg(tbx + bxt + 1);   // output nodes of the tile
         const int Ibeg = __ldg(tby + byt), Iend = __ldg(tby + byt + 1);
         const int offx = w0x & 3;
@@ -463,8 +467,21 @@ int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMa
     const long long n_tiles = (long long)grid.x * grid.y;
     if (n_tiles > 0x7fffffffLL) return 1;
     const unsigned ctas = (unsigned)n_tiles;
-    spline_tile_kernel<S><<<ctas, kTileThreads, S::smem_bytes, stream>>>(d_in, d_out, ax, ay, colw, rowtab, tbx, tby, rfirst, coli,
-                                                                          (int)grid.x, (int)n_tiles, 4 * kSMs /* CTAs resident at once */);
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(ctas);
+        cfg.blockDim = dim3(kTileThreads);
+        cfg.dynamicSmemBytes = S::smem_bytes;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        BATHY_CUDA_TRY(cudaLaunchKernelEx(&cfg, spline_tile_kernel<S>, d_in, d_out, ax, ay, (const float4*)colw, (const float4*)rowtab,
+                                          (const int*)tbx, (const int*)tby, (const int*)rfirst, (const int*)coli,
+                                          (int)grid.x, (int)n_tiles, 4 * kSMs /* CTAs resident at once */));
+    }
     count_launch(2);
     return launch_status();
 }
