@@ -263,7 +263,7 @@ def run_ours(args):
         st_b.synchronize(); st_s.synchronize(); st_k.synchronize()
         return float(hok[0, 0]) + float(hob[0, 0]) + float(hos[0, 0]) + int(hfail[0])      # the host reads the result
 
-    e2e_steps = max(2, min(args.steps, 5))
+    e2e_steps = max(2, min(args.steps, 10))
     e2e_step()
     barrier()
     te0 = time.perf_counter()
