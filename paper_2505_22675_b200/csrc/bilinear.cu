@@ -9,8 +9,8 @@
 // output row (nx_out = 8191 and 4093 are odd: rows are not 16-byte aligned, and a per-row shift to
 // float4 alignment would break the row-to-row register reuse below).  The thread marches down the TH
 // rows: the horizontal interpolants of the two bracketing input rows live in registers and are
-// recomputed only when the output row enters a new input interval, so a node costs one FMA, one
-// add and one store plus its share of the per-row and per-interval work.
+// recomputed only when the output row enters a new input interval, so a node costs half a packed FMA,
+// half a packed add (z_ref, added last) and one store plus its share of the per-row and per-interval work.
 #include "common.cuh"
 
 namespace bathy {
@@ -101,7 +101,7 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
     }
 
     // Two columns to a 64-bit register pair: a node is half a packed FMA (FFMA2) and a store.
-    u64 hlo2[CPT / 2], hd2[CPT / 2];                  // lower interpolant (+ z_ref) and (upper - lower)
+    u64 hlo2[CPT / 2], hd2[CPT / 2];                  // lower interpolant (relative to z_ref) and (upper - lower)
 #pragma unroll
     for (int p = 0; p < CPT / 2; ++p) hlo2[p] = hd2[p] = pack2(0.0f, 0.0f);
     int cur_j = -2;
@@ -148,7 +148,7 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
 #pragma unroll
             for (int p = 0; p < CPT / 2; ++p) {
                 hd2[p] = ffma2(lo2[p], neg1, hhi2[p]);
-                hlo2[p] = fadd2(lo2[p], cz2[p]);
+                hlo2[p] = lo2[p];
             }
             cur_j = j;
         }
@@ -156,14 +156,15 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
         if (full) {
 #pragma unroll
             for (int p = 0; p < CPT / 2; ++p) {
-                const u64 o = ffma2(s2, hd2[p], hlo2[p]);
+                // z_ref is added LAST: the only rounding at full magnitude (0.5 ulp of the depth)
+                const u64 o = fadd2(ffma2(s2, hd2[p], hlo2[p]), cz2[p]);
                 orow[64 * p] = lo_of(o);
                 orow[64 * p + 32] = hi_of(o);
             }
         } else {
 #pragma unroll
             for (int p = 0; p < CPT / 2; ++p) {
-                const u64 o = ffma2(s2, hd2[p], hlo2[p]);
+                const u64 o = fadd2(ffma2(s2, hd2[p], hlo2[p]), cz2[p]);
                 if (cok[2 * p]) orow[64 * p] = lo_of(o);
                 if (cok[2 * p + 1]) orow[64 * p + 32] = hi_of(o);
             }
@@ -186,9 +187,11 @@ bilinear_gather_kernel(const float* __restrict__ in, float* __restrict__ out, Ax
         if (i >= 0 && j >= 0) {
             const float* p = in + (size_t)j * ax.n_in + i;
             const float q11 = __ldg(p), q21 = __ldg(p + 1), q12 = __ldg(p + ax.n_in), q22 = __ldg(p + ax.n_in + 1);
-            const float lo = fmaf(t, q21 - q11, q11);
-            const float hi = fmaf(t, q22 - q12, q12);
-            f = fmaf(s, hi - lo, lo);
+            // on differences to q11, which is added last: one rounding at full magnitude
+            const float a = q21 - q11, b = q12 - q11, c = q22 - q11;
+            const float lo = t * a;
+            const float hi = fmaf(t, c - b, b);
+            f = q11 + fmaf(s, hi - lo, lo);
         }
         out[(size_t)I * ax.n_out + J] = f;
     }

@@ -22,8 +22,7 @@ def _check(z, gi, go):
     ref = oracle.catmull_rom(z, ogeom(gi), ogeom(go))
     got = _run(z, gi, go)
     err = max_abs_err(got, ref)                                       # also: identical NaN patterns
-    zr = float(np.nanmax(z) - np.nanmin(z))
-    assert err <= TOL * max(depth_range(ref), zr), (err, depth_range(ref))
+    assert err <= TOL * depth_range(ref), (err, depth_range(ref))
     return got, ref
 
 
@@ -72,12 +71,4 @@ def test_quadratic_exact_and_knots():
     assert np.array_equal(got[::4, ::4], z[1:39, 1:49][: got[::4, ::4].shape[0], : got[::4, ::4].shape[1]])   # knots bit-exact
 
 
-def test_full_size_config3_sampled_rows():
-    w = W.grid_config(3)
-    gi, go = w.geom_in, w.geom_out
-    got = _run(w.z, gi, go)
-    assert np.isfinite(got).all()
-    stride = (go.ny - 1) // 5
-    sub = W.Geom(go.nx, 6, go.x0, go.y0, go.dx, go.dy * stride)
-    ref = oracle.catmull_rom(w.z, ogeom(gi), ogeom(sub))
-    assert np.abs(got[np.arange(6) * stride, :] - ref).max() <= TOL * float(w.z.max() - w.z.min())
+# (full-size config 2 / config 3 parity on EVERY node: tests/test_gpu_full_size.py)
