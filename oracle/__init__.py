@@ -36,7 +36,7 @@ class Vgm(C.Structure):
     _fields_ = [("model", C.c_int32), ("range", C.c_double), ("sill", C.c_double), ("nugget", C.c_double)]
 
 
-EXPONENTIAL, SPHERICAL = 0, 1
+EXPONENTIAL, SPHERICAL, GAUSSIAN = 0, 1, 2
 _lib = None
 
 
@@ -69,6 +69,9 @@ def lib():
         L.oracle_krige_points.argtypes = [fp, fp, fp, C.c_int64, C.c_void_p, fp, fp, C.c_int64, vp,
                                           C.c_int, dp, ip, dp]
         L.oracle_krige_points.restype = C.c_int64
+        L.oracle_krige_points_var.argtypes = [fp, fp, fp, C.c_int64, C.c_void_p, fp, fp, C.c_int64, vp,
+                                              C.c_int, dp, dp, ip]
+        L.oracle_krige_points_var.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -222,8 +225,10 @@ def ok_weights(px, py, xq, yq, v: Vgm):
 
 
 def krige_points(x, y, z, xq, yq, v: Vgm, k: int, buckets: Buckets | None = None,
-                 want_nbr: bool = True, want_lambda: bool = False):
-    """K1-K5 at fp32 query points.  Returns dict(zhat float64 [nq], nbr int32 [nq,k], lam, failed)."""
+                 want_nbr: bool = True, want_lambda: bool = False, want_var: bool = False):
+    """K1-K5 at fp32 query points.  Returns dict(zhat float64 [nq], nbr int32 [nq,k], lam, failed[, var])."""
+    if want_var:
+        return _krige_points_var(x, y, z, xq, yq, v, k, buckets, want_nbr)
     x, y, z = _f32(x), _f32(y), _f32(z)
     xq, yq = _f32(np.ravel(xq)), _f32(np.ravel(yq))
     nq = xq.shape[0]
@@ -241,11 +246,30 @@ def krige_points(x, y, z, xq, yq, v: Vgm, k: int, buckets: Buckets | None = None
     return {"zhat": zhat, "nbr": nbr, "lam": lam, "failed": int(failed)}
 
 
+def _krige_points_var(x, y, z, xq, yq, v, k, buckets, want_nbr):
+    x, y, z = _f32(x), _f32(y), _f32(z)
+    xq, yq = _f32(np.ravel(xq)), _f32(np.ravel(yq))
+    nq = xq.shape[0]
+    zhat = np.empty(nq, dtype=np.float64)
+    var = np.empty(nq, dtype=np.float64)
+    nbr = np.empty((nq, k), dtype=np.int32) if want_nbr else None
+    failed = lib().oracle_krige_points_var(
+        _p(x, C.c_float), _p(y, C.c_float), _p(z, C.c_float), x.shape[0],
+        buckets.h if buckets is not None else None,
+        _p(xq, C.c_float), _p(yq, C.c_float), nq, C.byref(v), int(k),
+        _p(zhat, C.c_double), _p(var, C.c_double), _p(nbr, C.c_int32) if want_nbr else None)
+    if failed < 0:
+        raise ValueError(f"oracle_krige_points_var: {failed}")
+    return {"zhat": zhat, "var": var, "nbr": nbr, "lam": None, "failed": int(failed)}
+
+
 def krige_grid(x, y, z, g: Geom, v: Vgm, k: int, buckets: Buckets | None = None, **kw):
     """Kriging onto every node of grid g (node coordinates per K1)."""
     xq, yq = node_coords(g)
     r = krige_points(x, y, z, xq, yq, v, k, buckets, **kw)
     r["zhat"] = r["zhat"].reshape(g.ny, g.nx)
+    if r.get("var") is not None:
+        r["var"] = r["var"].reshape(g.ny, g.nx)
     if r["nbr"] is not None:
         r["nbr"] = r["nbr"].reshape(g.ny, g.nx, k)
     return r

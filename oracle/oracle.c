@@ -14,7 +14,8 @@
  * 0.47265625, M=(0,18/7,-30/7,18/7,0), scipy CubicSpline(natural), two-point closed form
  * lambda1=0.748755187238, equilateral 1/3, constants, sum(lambda)=1, exactness at data, brute-force
  * kNN vs bucket kNN, LU vs numpy.linalg.solve; Catmull-Rom: C(0)=P1, C(1)=P2, C(1/2)=(-P0+9P1+9P2-P3)/16,
- * quadratics reproduced, NaN/edge fallback = bilinear.  No function here is "parity unpinned" against
+ * quadratics reproduced, NaN/edge fallback = bilinear; kriging variance: two-point closed form 0.148703758152,
+ * zero at data, sill (1 + 1/k) for the local mean, C-form LAPACK; Gaussian variogram gamma(a).  No function here is "parity unpinned" against
  * mathematics; nothing is pinned against the paper's own tables (they need GEBCO).
  */
 #include <math.h>
@@ -30,7 +31,8 @@
 typedef struct { int32_t nx, ny; float x0, y0, dx, dy; } ora_geom;
 
 /* Variogram: model 0 = exponential exactly as PAPER.md:L157 (no factor 3), 1 = spherical
- * (textbook).  sill is the TOTAL sill; c_p = sill - nugget.  gamma(0) = 0 exactly. */
+ * (textbook), 2 = Gaussian (textbook, same no-factor-3 convention).
+ * sill is the TOTAL sill; c_p = sill - nugget.  gamma(0) = 0 exactly. */
 typedef struct { int32_t model; double range, sill, nugget; } ora_vgm;
 
 int oracle_num_threads(void)
@@ -435,12 +437,14 @@ int oracle_knn_buckets(const ora_buckets *b, const float *x, const float *y, flo
 /* K3: variogram.  Exponential exactly as printed at PAPER.md:L157, gamma(h) = C0 (1 - exp(-h/a)),
  * extended by a nugget the textbook way: gamma(h) = nugget + c_p (1 - exp(-h/a)), c_p = sill -
  * nugget, for h > 0.  Spherical (textbook): nugget + c_p (1.5 h/a - 0.5 (h/a)^3) for 0 < h < a,
- * sill for h >= a.  gamma(0) = 0 exactly for both. */
+ * sill for h >= a.  Gaussian (textbook, NEXT-4): nugget + c_p (1 - exp(-(h/a)^2)).  gamma(0) = 0 exactly
+ * for all three. */
 double oracle_variogram(const ora_vgm *v, double h)
 {
     if (h == 0.0) return 0.0;
     double cp = v->sill - v->nugget;
     if (v->model == 0) return v->nugget + cp * (1.0 - exp(-h / v->range));
+    if (v->model == 2) return v->nugget + cp * (1.0 - exp(-(h / v->range) * (h / v->range)));
     if (h >= v->range) return v->sill;
     double q = h / v->range;
     return v->nugget + cp * (1.5 * q - 0.5 * q * q * q);
@@ -514,15 +518,15 @@ int oracle_ok_weights(const double *px, const double *py, int k, double xq, doub
  * nbr_out [nq*k] (or NULL) receives original indices in ascending (key, index) order;
  * lambda_out [nq*k] (or NULL) the weights in the same order.  A singular node gets NaN.
  * Returns the number of singular nodes, or a negative error. */
-int64_t oracle_krige_points(const float *x, const float *y, const float *z, int64_t n,
+static int64_t krige_points_impl(const float *x, const float *y, const float *z, int64_t n,
                             const ora_buckets *buckets,
                             const float *xq, const float *yq, int64_t nq,
                             const ora_vgm *v, int k,
-                            double *zhat, int32_t *nbr_out, double *lambda_out)
+                            double *zhat, int32_t *nbr_out, double *lambda_out, double *var_out)
 {
     if (!x || !y || !z || !xq || !yq || !zhat || k < 1 || k > n || k > 4096) return -1;
     if (!(v->range > 0.0) || !(v->sill > 0.0) || v->nugget < 0.0 || v->nugget > v->sill) return -1;
-    if (v->model != 0 && v->model != 1) return -1;
+    if (v->model != 0 && v->model != 1 && v->model != 2) return -1;
     int64_t failed = 0;
     #pragma omp parallel for schedule(dynamic, 64) reduction(+:failed)
     for (int64_t q = 0; q < nq; ++q) {
@@ -530,21 +534,48 @@ int64_t oracle_krige_points(const float *x, const float *y, const float *z, int6
         double px[4096], py[4096], lam[4096];
         int rc = buckets ? oracle_knn_buckets(buckets, x, y, xq[q], yq[q], k, idx, NULL)
                          : oracle_knn_brute(x, y, n, xq[q], yq[q], k, idx, NULL);
-        double est = NAN;
+        double est = NAN, var = NAN, mu = 0.0;
         if (rc == 0) {
             for (int i = 0; i < k; ++i) { px[i] = (double)x[idx[i]]; py[i] = (double)y[idx[i]]; }
-            rc = oracle_ok_weights(px, py, k, (double)xq[q], (double)yq[q], v, lam, NULL);
+            rc = oracle_ok_weights(px, py, k, (double)xq[q], (double)yq[q], v, lam, &mu);
         }
         if (rc == 0) {
             est = 0.0;
             for (int i = 0; i < k; ++i) est += lam[i] * (double)z[idx[i]];
+            /* ordinary-kriging variance (textbook, e.g. Cressie, the paper's ref [4]):
+             * sigma^2 = sum_i lambda_i gamma(|q - p_i|) + mu, mu the Lagrange multiplier of the gamma form */
+            var = mu;
+            for (int i = 0; i < k; ++i) {
+                double dx = (double)xq[q] - px[i], dy = (double)yq[q] - py[i];
+                var += lam[i] * oracle_variogram(v, sqrt(dx * dx + dy * dy));
+            }
         } else {
             failed += 1;
             for (int i = 0; i < k; ++i) lam[i] = NAN;
         }
         zhat[q] = est;
+        if (var_out) var_out[q] = var;
         if (nbr_out) for (int i = 0; i < k; ++i) nbr_out[q * k + i] = idx[i];
         if (lambda_out) for (int i = 0; i < k; ++i) lambda_out[q * k + i] = lam[i];
     }
     return failed;
+}
+
+int64_t oracle_krige_points(const float *x, const float *y, const float *z, int64_t n,
+                            const ora_buckets *buckets,
+                            const float *xq, const float *yq, int64_t nq,
+                            const ora_vgm *v, int k,
+                            double *zhat, int32_t *nbr_out, double *lambda_out)
+{
+    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, k, zhat, nbr_out, lambda_out, NULL);
+}
+
+/* The same with the kriging variance sigma^2 in var_out [nq]. */
+int64_t oracle_krige_points_var(const float *x, const float *y, const float *z, int64_t n,
+                                const ora_buckets *buckets,
+                                const float *xq, const float *yq, int64_t nq,
+                                const ora_vgm *v, int k,
+                                double *zhat, double *var_out, int32_t *nbr_out)
+{
+    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, k, zhat, nbr_out, NULL, var_out);
 }

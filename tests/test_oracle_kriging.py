@@ -277,3 +277,72 @@ def test_krige_argument_errors():
             oracle.krige_points(x, x, x, [0.0], [0.0], bad, 2)
     with pytest.raises(ValueError):
         oracle.krige_points(x, x, x, [0.0], [0.0], oracle.vgm(EXP, 1, 1, 0), 4)     # k > n
+
+
+# ---------------------------------------------------------------- NEXT-3: kriging variance; NEXT-4: Gaussian model
+
+def test_variance_two_point_closed_form():
+    """sigma^2 = sum lambda_i gamma_i0 + mu.  Two points: rows of the gamma form give gamma12 lambda2 + mu = gamma1,
+    so mu = gamma1 - gamma12 lambda2 with lambda1 = 1/2 + (gamma2 - gamma1)/(2 gamma12) -- retyped here in numpy,
+    and the value SURVEY.md 8(c) prints for (0,0),(4,0), query (1,0), exponential a=10, sill 1: 0.148703758152."""
+    x, y, z = np.array([0, 4], np.float32), np.array([0, 0], np.float32), np.array([10, 20], np.float32)
+    for model, gam in ((oracle.EXPONENTIAL, lambda h: 1 - np.exp(-h / 10.0)), (oracle.GAUSSIAN, lambda h: 1 - np.exp(-(h / 10.0) ** 2)),
+                       (oracle.SPHERICAL, lambda h: 1.5 * h / 10 - 0.5 * (h / 10) ** 3)):
+        g1, g2, g12 = gam(1.0), gam(3.0), gam(4.0)
+        l1 = 0.5 + (g2 - g1) / (2 * g12)
+        mu = g1 - g12 * (1 - l1)
+        want = l1 * g1 + (1 - l1) * g2 + mu
+        r = oracle.krige_points(x, y, z, [1.0], [0.0], oracle.vgm(model, 10.0, 1.0, 0.0), 2, want_var=True)
+        assert abs(r["var"][0] - want) < 1e-13 and abs(r["zhat"][0] - (l1 * 10 + (1 - l1) * 20)) < 1e-12
+        if model == oracle.EXPONENTIAL:
+            assert abs(r["var"][0] - 0.148703758152) < 1e-11
+
+
+def test_variance_zero_at_data_local_mean_and_scaling():
+    rng = np.random.default_rng(5)
+    x, y = rng.uniform(0, 50, 40).astype(np.float32), rng.uniform(0, 50, 40).astype(np.float32)
+    z = rng.normal(-100, 3, 40).astype(np.float32)
+    v = oracle.vgm(oracle.EXPONENTIAL, 15.0, 4.0, 0.4)
+    r = oracle.krige_points(x, y, z, x[:5], y[:5], v, 8, want_var=True)
+    assert np.abs(r["var"]).max() < 1e-12                         # gamma(0) = 0: no error at a datum
+    r = oracle.krige_points(x, y, z, [3.3, 41.0], [7.7, 20.0], v, 8, want_var=True)
+    assert (r["var"] > 0).all() and (r["var"] < 2 * 4.0).all()
+    # sigma^2 scales with (sill, nugget) -> alpha (sill, nugget); the estimate does not
+    r2 = oracle.krige_points(x, y, z, [3.3, 41.0], [7.7, 20.0], oracle.vgm(oracle.EXPONENTIAL, 15.0, 12.0, 1.2), 8, want_var=True)
+    assert np.allclose(r2["var"], 3 * r["var"], rtol=1e-12) and np.allclose(r2["zhat"], r["zhat"], rtol=1e-13)
+    # all k neighbours mutually and from the node beyond a spherical range: lambda = 1/k, mu = sill/k,
+    # sigma^2 = sill (1 + 1/k)
+    xs, ys = np.array([0, 100, 0, 100], np.float32), np.array([0, 0, 100, 100], np.float32)
+    r = oracle.krige_points(xs, ys, np.array([1, 2, 3, 4], np.float32), [50.0], [50.0], oracle.vgm(oracle.SPHERICAL, 10.0, 2.0, 0.5), 4, want_var=True)
+    assert abs(r["var"][0] - 2.0 * 1.25) < 1e-12 and abs(r["zhat"][0] - 2.5) < 1e-12
+
+
+@pytest.mark.parametrize("model", [oracle.EXPONENTIAL, oracle.SPHERICAL, oracle.GAUSSIAN])
+def test_variance_vs_c_form_lapack(model):
+    """C-form with LAPACK: [C 1; 1^T 0][lambda; mu_C] = [c0; 1], sigma^2 = sill - lambda.c0 - mu_C."""
+    rng = np.random.default_rng(17 + model)
+    k = 6
+    x, y = rng.uniform(0, 20, k).astype(np.float32), rng.uniform(0, 20, k).astype(np.float32)
+    z = rng.normal(0, 1, k).astype(np.float32)
+    sill, nug, a = 3.0, 0.3, 9.0
+    v = oracle.vgm(model, a, sill, nug)
+    xq, yq = np.float32(8.5), np.float32(11.25)
+    r = oracle.krige_points(x, y, z, [xq], [yq], v, k, want_var=True)
+    xd, yd = x.astype(np.float64), y.astype(np.float64)
+    H = np.hypot(xd[:, None] - xd[None, :], yd[:, None] - yd[None, :])
+    h0 = np.hypot(xd - float(xq), yd - float(yq))
+    cov = lambda h: np.where(h == 0, sill, sill - oracle.variogram(v, h.ravel()).reshape(h.shape))
+    A = np.zeros((k + 1, k + 1)); A[:k, :k] = cov(H); A[:k, k] = A[k, :k] = 1.0
+    b = np.append(cov(h0), 1.0)
+    sol = np.linalg.solve(A, b)
+    want = sill - sol[:k] @ b[:k] - sol[k]
+    assert abs(r["var"][0] - want) < 1e-10 and abs(r["zhat"][0] - sol[:k] @ z.astype(np.float64)) < 1e-10
+
+
+def test_gaussian_variogram_values():
+    v = oracle.vgm(oracle.GAUSSIAN, 8.0, 5.0, 1.0)
+    g = oracle.variogram(v, [0.0, 8.0, 1e-300, 4.0, 1e6])
+    assert g[0] == 0.0                                            # gamma(0) = 0 with a nugget
+    assert abs(g[1] - (1.0 + 4.0 * (1 - np.exp(-1.0)))) < 1e-14   # gamma(a) = nugget + c_p (1 - 1/e)
+    assert abs(g[2] - 1.0) < 1e-14 and abs(g[3] - (1.0 + 4.0 * (1 - np.exp(-0.25)))) < 1e-14
+    assert abs(g[4] - 5.0) < 1e-14
