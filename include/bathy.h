@@ -9,12 +9,17 @@
  *     The library never allocates or frees caller buffers and never keeps a caller pointer after
  *     the call's work on `cuda_stream` has completed.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-
- *     pointer calls are asynchronous on that stream and do not synchronise the host.  `*_host`
- *     calls copy host->device, run the same kernels and copy device->host on that stream and
- *     return after the stream has drained.
+ *     pointer calls only ENQUEUE work on that stream and never synchronise the host (the two
+ *     exceptions say so: krige_index_info and krige_free_index).  `*_host` calls copy host->device,
+ *     run the same kernels and copy device->host on that stream and return after the stream has
+ *     drained; `*_host_async` calls only enqueue.
  *   - Return value: 0 (BATHY_OK) or a negative bathy_status.  Argument errors are detected
- *     synchronously and nothing is launched.  No exceptions, no global state besides the launch
- *     counter, no environment variables; calls on distinct streams are thread-safe.
+ *     synchronously and nothing is launched.  No exceptions, no environment variables.  Global state:
+ *     the launch counter, the spline path selector, and per-DEVICE one-time setup (kernel attributes;
+ *     the first index call on a device raises the release threshold of that device's default memory
+ *     pool to 2 GiB so that stream-ordered scratch is recycled instead of returned to the driver).
+ *     Calls on distinct streams are thread-safe, and one process may use several devices (the current
+ *     device of the calling thread is used; an index belongs to the device it was built on).
  *   - A grid is row-major fp32 with leading dimension nx.  Node (i, j) -- i = row (y), j = column
  *     (x) -- sits at x = x0 + j*dx, y = y0 + i*dy.
  *   - There is no CPU fallback: without a CUDA device every compute call returns BATHY_ERR_CUDA.
@@ -67,6 +72,9 @@ typedef struct {
 
 #define BATHY_VGM_EXPONENTIAL 0
 #define BATHY_VGM_SPHERICAL   1
+/* SURVEY.md 8(f) NEXT-4 ("many variants ... can be easily implemented on top"): Gaussian,
+ * gamma(h) = nugget + (sill-nugget)(1 - exp(-(h/range)^2)) in the same no-factor-3 convention as L157. */
+#define BATHY_VGM_GAUSSIAN    2
 
 /* Opaque, library-owned, immutable after build; may be shared by concurrent krige_predict calls. */
 typedef struct krige_index krige_index_t;
@@ -114,10 +122,15 @@ BATHY_API int interp_spline(const float* d_in, grid_geom_t in, float* d_out, gri
  * cell id per sounding, histogram, exclusive scan, stable scatter of (x, y, z, original index).
  * d_x, d_y, d_z [n] fp32 (SoA), n in [1, 2^31-1]; finite, no two soundings at identical (x, y)
  * (kriging with duplicates is singular -- such nodes come out NaN, see krige_predict).
- * cell_size: edge of a square cell in the units of x/y; 0 = automatic (about 8 soundings per cell).
+ * cell_size: edge of a square cell in the units of x/y; 0 = automatic (about 8 soundings per cell).  A
+ * performance knob only: results do not depend on it.  The library enlarges it when the cell grid would
+ * exceed 4 cells per sounding or 2^26 cells.
  * The soundings are copied into library-owned device memory: the caller may free d_x/d_y/d_z once
- * the stream reaches this point.  The call synchronises `cuda_stream` once (to size the cell
- * grid from the bounding box).  *out_index is released only by krige_free_index. */
+ * the stream reaches this point.  ENQUEUE ONLY: the bounding box never comes back to the host -- the
+ * cell grid is sized by a kernel and lives in a device header that krige_predict reads.  Non-finite
+ * coordinates therefore cannot be reported by this call: they mark the index unusable on the device,
+ * krige_index_info then returns BATHY_ERR_GEOMETRY and every krige_predict node comes out NaN and is
+ * counted in d_failed.  *out_index is released only by krige_free_index[_async]. */
 BATHY_API int krige_build_index(const float* d_x, const float* d_y, const float* d_z, int64_t n,
                       float cell_size, void* cuda_stream, krige_index_t** out_index);
 
@@ -143,7 +156,9 @@ BATHY_API int krige_build_index(const float* d_x, const float* d_y, const float*
 BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram_t vg, int32_t k,
                   float* d_zhat, int32_t* d_nbr_or_null, int64_t* d_failed_or_null, void* cuda_stream);
 
-/* Releases an index (synchronises the device first).  NULL is a no-op. */
+/* Releases an index after synchronising the stream of its last build / append (NOT the device): the
+ * caller guarantees that every krige_predict that uses it was issued on that stream or has completed.
+ * NULL is a no-op. */
 BATHY_API void krige_free_index(krige_index_t* idx);
 
 /* Stream-ordered release, no host synchronisation: the index memory returns to the device's memory
@@ -153,9 +168,51 @@ BATHY_API void krige_free_index(krige_index_t* idx);
  * release -- without ever stalling the host.) */
 BATHY_API void krige_free_index_async(krige_index_t* idx, void* cuda_stream);
 
-/* Introspection of an index (host values, valid after build): number of soundings, cell size used,
- * cell-grid dimensions. */
+/* Introspection of an index: number of soundings, cell size used, cell-grid dimensions.  These live on
+ * the device, so this call WAITS for the stream of the last build / append.  Returns BATHY_ERR_GEOMETRY
+ * when the soundings held a non-finite coordinate. */
 BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell_size, int32_t* ncx, int32_t* ncy);
+
+/* ---------------------------------------------------------------------------------------------
+ * krige_predict_ex -- krige_predict with optional extra outputs.  All pointers
+ * may be NULL; `outputs_or_null` == NULL is krige_predict without neighbour and failure outputs.
+ *   d_var      [out.ny * out.nx] fp32: the ordinary-kriging variance
+ *              sigma^2 = sum_i lambda_i gamma(h_0i) + mu   (mu: the Lagrange multiplier of the gamma-form
+ *              system [Gamma 1; 1^T 0][lambda; mu] = [gamma0; 1], the standard form of PAPER.md:L159-L165),
+ *              in the units of sill; 0 at a node that coincides with a sounding; NaN where the node failed.
+ *   d_nbr, d_failed: as krige_predict.
+ *   d_illcond  one int64 device counter, INCREMENTED by the number of nodes whose smallest Cholesky pivot
+ *              of the sill-normalised covariance matrix fell below BATHY_ILLCOND_PIVOT (neighbours much
+ *              closer to each other than the variogram range): their estimate is finite but the fp32
+ *              factorisation has lost accuracy, relative error of the weights ~ k * 6e-8 / pivot
+ *              (reading K-cond).  The caller zeroes it. */
+typedef struct {
+    float*   d_var;
+    int32_t* d_nbr;
+    int64_t* d_failed;
+    int64_t* d_illcond;
+} krige_outputs_t;
+#define BATHY_ILLCOND_PIVOT 1e-3f
+BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variogram_t vg, int32_t k,
+                     float* d_zhat, const krige_outputs_t* outputs_or_null, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Streaming index (the paper's real-time onboard goal).
+ * krige_index_create makes an EMPTY index over the caller's extent -- the planned survey area
+ * [xmin, xmax] x [ymin, ymax]; soundings outside it are legal and are kept in the border cells -- with
+ * room for `capacity` soundings; krige_index_append merges a batch of n soundings (the pings that just
+ * arrived) into it.  The original index of a sounding is its position in the concatenation of all
+ * appended batches.  create + append(A) + append(B) gives bit for bit the index of create + append(A|B),
+ * hence identical neighbours and depths.  Both calls only enqueue work.  Appends and the krige_predict
+ * calls that use the index must be ordered by the caller (same stream, or events): an append rewrites the
+ * buffers the append before it read from.  After an append only nodes within their k-th-neighbour
+ * distance of the new soundings change: d_changed_bbox_or_null (4 floats on the device: xmin, xmax,
+ * ymin, ymax of the batch) tells the caller which tiles to predict again.
+ * Errors: BATHY_ERR_SIZE (capacity exceeded, n < 1), BATHY_ERR_INDEX (index not made by krige_index_create). */
+BATHY_API int krige_index_create(float xmin, float xmax, float ymin, float ymax, float cell_size, int64_t capacity,
+                       void* cuda_stream, krige_index_t** out_index);
+BATHY_API int krige_index_append(krige_index_t* idx, const float* d_x, const float* d_y, const float* d_z, int64_t n,
+                       float* d_changed_bbox_or_null, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Host-buffer forms: the same operations for callers whose data lives in host memory.  Each
@@ -164,13 +221,13 @@ BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell
  * the copies asynchronous and faster but is not required. */
 BATHY_API int interp_bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
 BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
+BATHY_API int interp_catmull_rom_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
 BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
                grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
                void* cuda_stream);
 
 /* The same three, ENQUEUED only: scratch allocation, copies, kernels and releases are all ordered on
- * `cuda_stream` and the call returns without waiting for them (krige_host_async waits once, on its
- * own stream, for the soundings' bounding box -- see krige_build_index).  The host buffers must be
+ * `cuda_stream` and the call returns without waiting for them.  The host buffers must be
  * pinned (otherwise the copies fall back to synchronous staging) and must stay valid, and h_out /
  * h_zhat / *h_failed_or_null are defined, only after the caller has synchronised `cuda_stream`.
  * Issued on different streams, the copies of one call overlap the kernels and the opposite-direction
@@ -179,6 +236,7 @@ BATHY_API int krige_host(const float* h_x, const float* h_y, const float* h_z, i
  * caller's synchronisation. */
 BATHY_API int interp_bilinear_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
 BATHY_API int interp_spline_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
+BATHY_API int interp_catmull_rom_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream);
 BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* h_z, int64_t n, float cell_size,
                grid_geom_t out, variogram_t vg, int32_t k, float* h_zhat, int64_t* h_failed_or_null,
                void* cuda_stream);
@@ -189,7 +247,7 @@ BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* 
  * 1 = fused tile kernel only (BATHY_ERR_GEOMETRY where it does not apply);
  * 2 = global-solve path only (three batched full-length Thomas solves + gather evaluate).
  * Both compute the same natural bicubic spline; DESIGN.md "Spline window bound" gives the bound on
- * their difference (2.2e-7 x depth range). */
+ * their difference (8.2e-7 x depth range per direction). */
 BATHY_API int bathy_set_spline_path(int path);
 
 /* Static, never NULL. */

@@ -18,13 +18,15 @@ from .workloads import Geom
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbathy.so")
 
-EXPONENTIAL, SPHERICAL = 0, 1
+EXPONENTIAL, SPHERICAL, GAUSSIAN = 0, 1, 2
 MAX_K = 64
 
 SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_bytes", "interp_spline", "krige_build_index",
            "krige_predict", "krige_free_index", "krige_free_index_async", "krige_index_info", "interp_bilinear_host",
            "interp_spline_host", "krige_host", "interp_bilinear_host_async", "interp_spline_host_async",
-           "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path"]
+           "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path",
+           "krige_predict_ex", "krige_index_create", "krige_index_append", "interp_catmull_rom_host",
+           "interp_catmull_rom_host_async"]
 
 
 class GridGeom(C.Structure):
@@ -34,6 +36,10 @@ class GridGeom(C.Structure):
 
 class Variogram(C.Structure):
     _fields_ = [("model", C.c_int32), ("range", C.c_float), ("sill", C.c_float), ("nugget", C.c_float)]
+
+
+class KrigeOutputs(C.Structure):
+    _fields_ = [("d_var", C.c_void_p), ("d_nbr", C.c_void_p), ("d_failed", C.c_void_p), ("d_illcond", C.c_void_p)]
 
 
 class BathyError(RuntimeError):
@@ -61,6 +67,9 @@ def lib():
         L.interp_spline.argtypes = [vp, GridGeom, vp, GridGeom, vp, C.c_size_t, vp]
         L.krige_build_index.argtypes = [vp, vp, vp, C.c_int64, C.c_float, vp, C.POINTER(vp)]
         L.krige_predict.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, vp, vp, vp]
+        L.krige_predict_ex.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, C.POINTER(KrigeOutputs), vp]
+        L.krige_index_create.argtypes = [C.c_float] * 5 + [C.c_int64, vp, C.POINTER(vp)]
+        L.krige_index_append.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
         L.krige_free_index.argtypes = [vp]
         L.krige_free_index.restype = None
         L.krige_free_index_async.argtypes = [vp, vp]
@@ -70,6 +79,8 @@ def lib():
         L.interp_bilinear_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
         L.interp_spline_host.argtypes = [vp, GridGeom, vp, GridGeom, vp]
         L.krige_host.argtypes = [vp, vp, vp, C.c_int64, C.c_float, GridGeom, Variogram, C.c_int32, vp, vp, vp]
+        L.interp_catmull_rom_host.argtypes = L.interp_bilinear_host.argtypes
+        L.interp_catmull_rom_host_async.argtypes = L.interp_bilinear_host.argtypes
         L.interp_bilinear_host_async.argtypes = L.interp_bilinear_host.argtypes
         L.interp_spline_host_async.argtypes = L.interp_spline_host.argtypes
         L.krige_host_async.argtypes = L.krige_host.argtypes
@@ -153,9 +164,12 @@ def interp_spline(z: torch.Tensor, gin, gout, out: torch.Tensor | None = None,
     if out is None:
         out = torch.empty((go.ny, go.nx), dtype=torch.float32, device=z.device)
     _dev_f32(out, "out")
+    assert out.numel() == go.nx * go.ny
     need = interp_spline_workspace_bytes(gi, go)
     if workspace is None:
         workspace = torch.empty(need, dtype=torch.uint8, device=z.device)
+        if stream is not None and hasattr(workspace, "record_stream") and hasattr(stream, "cuda_stream"):
+            workspace.record_stream(stream)            # the temporary outlives this call on `stream`
     _check(lib().interp_spline(z.data_ptr(), gi, out.data_ptr(), go, workspace.data_ptr(),
                                workspace.numel() * workspace.element_size(), _stream(stream)), "interp_spline")
     return out
@@ -201,21 +215,72 @@ def krige_build_index(x: torch.Tensor, y: torch.Tensor, z: torch.Tensor, cell_si
     return KrigeIndex(h.value)
 
 
+def _counter(t, name):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.int64 and t.numel() == 1):
+        raise TypeError(f"{name} must be an int64 CUDA tensor of one element")
+    return t.data_ptr()
+
+
 def krige_predict(index: KrigeIndex, gout, model: int, range_: float, sill: float, nugget: float, k: int,
                   out: torch.Tensor | None = None, want_nbr: bool = False, failed: torch.Tensor | None = None,
-                  stream=None):
-    """PAPER.md:L146-L171.  Returns zhat [ny, nx] (and nbr [ny, nx, k] int32 when want_nbr)."""
+                  stream=None, want_var: bool = False, var: torch.Tensor | None = None,
+                  illcond: torch.Tensor | None = None):
+    """PAPER.md:L146-L171.  Returns zhat [ny, nx]; with want_nbr also nbr [ny, nx, k] int32; with want_var (or
+    `var`) also the kriging variance [ny, nx] (krige_predict_ex): (zhat[, nbr][, var])."""
     go = _geom(gout)
     dev = torch.device("cuda", torch.cuda.current_device())
     if out is None:
         out = torch.empty((go.ny, go.nx), dtype=torch.float32, device=dev)
     _dev_f32(out, "out")
+    if out.numel() != go.nx * go.ny:
+        raise ValueError("out has the wrong number of elements")
     nbr = torch.empty((go.ny, go.nx, int(k)), dtype=torch.int32, device=dev) if want_nbr else None
+    if var is None and want_var:
+        var = torch.empty((go.ny, go.nx), dtype=torch.float32, device=dev)
+    if var is not None:
+        _dev_f32(var, "var")
+        if var.numel() != go.nx * go.ny:
+            raise ValueError("var has the wrong number of elements")
+    if stream is not None and hasattr(stream, "cuda_stream"):
+        for t in (nbr, var):
+            if t is not None:
+                t.record_stream(stream)
     vg = Variogram(int(model), float(range_), float(sill), float(nugget))
-    _check(lib().krige_predict(index.handle, go, vg, int(k), out.data_ptr(),
-                               nbr.data_ptr() if nbr is not None else None,
-                               failed.data_ptr() if failed is not None else None, _stream(stream)), "krige_predict")
-    return (out, nbr) if want_nbr else out
+    fp, ip = _counter(failed, "failed"), _counter(illcond, "illcond")
+    if var is None and ip is None:
+        _check(lib().krige_predict(index.handle, go, vg, int(k), out.data_ptr(),
+                                   nbr.data_ptr() if nbr is not None else None, fp, _stream(stream)), "krige_predict")
+    else:
+        outs = KrigeOutputs(var.data_ptr() if var is not None else None, nbr.data_ptr() if nbr is not None else None, fp, ip)
+        _check(lib().krige_predict_ex(index.handle, go, vg, int(k), out.data_ptr(), C.byref(outs), _stream(stream)),
+               "krige_predict_ex")
+    res = (out,) + ((nbr,) if want_nbr else ()) + ((var,) if var is not None else ())
+    return res if len(res) > 1 else out
+
+
+def krige_index_create(xmin: float, xmax: float, ymin: float, ymax: float, capacity: int, cell_size: float = 0.0,
+                       stream=None) -> KrigeIndex:
+    """an empty, appendable index over the planned survey extent (include/bathy.h)."""
+    h = C.c_void_p()
+    _check(lib().krige_index_create(float(xmin), float(xmax), float(ymin), float(ymax), float(cell_size), int(capacity),
+                                    _stream(stream), C.byref(h)), "krige_index_create")
+    return KrigeIndex(h.value)
+
+
+def krige_index_append(index: KrigeIndex, x: torch.Tensor, y: torch.Tensor, z: torch.Tensor,
+                       changed: torch.Tensor | None = None, stream=None) -> None:
+    """Merges a batch of soundings into an appendable index; `changed` (4 floats on the GPU) receives the
+    batch's bounding box xmin, xmax, ymin, ymax."""
+    for t, nm in ((x, "x"), (y, "y"), (z, "z")):
+        _dev_f32(t, nm)
+    assert x.numel() == y.numel() == z.numel()
+    if changed is not None:
+        _dev_f32(changed, "changed")
+        assert changed.numel() == 4
+    _check(lib().krige_index_append(index.handle, x.data_ptr(), y.data_ptr(), z.data_ptr(), x.numel(),
+                                    changed.data_ptr() if changed is not None else None, _stream(stream)), "krige_index_append")
 
 
 def krige_free_index(index: KrigeIndex) -> None:
@@ -233,13 +298,34 @@ def _host_f32(a, name):
     return a, a.ctypes.data
 
 
+def _host_out_f32(a, go):
+    """A caller-supplied host OUTPUT must be written in place: contiguous float32 of the right size."""
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous() or a.numel() != go.nx * go.ny:
+            raise TypeError("out must be a contiguous float32 host tensor with ny*nx elements")
+        return a, a.data_ptr()
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags["C_CONTIGUOUS"] and a.size == go.nx * go.ny):
+        raise TypeError("out must be a C-contiguous float32 numpy array with ny*nx elements")
+    return a, a.ctypes.data
+
+
 def interp_bilinear_host(z, gin, gout, out=None, stream=None):
     gi, go = _geom(gin), _geom(gout)
     z, zp = _host_f32(z, "z")
     if out is None:
         out = np.empty((go.ny, go.nx), dtype=np.float32)
-    out, op = _host_f32(out, "out")
+    out, op = _host_out_f32(out, go)
     _check(lib().interp_bilinear_host(zp, gi, op, go, _stream(stream)), "interp_bilinear_host")
+    return out
+
+
+def interp_catmull_rom_host(z, gin, gout, out=None, stream=None):
+    gi, go = _geom(gin), _geom(gout)
+    z, zp = _host_f32(z, "z")
+    if out is None:
+        out = np.empty((go.ny, go.nx), dtype=np.float32)
+    out, op = _host_out_f32(out, go)
+    _check(lib().interp_catmull_rom_host(zp, gi, op, go, _stream(stream)), "interp_catmull_rom_host")
     return out
 
 
@@ -248,7 +334,7 @@ def interp_spline_host(z, gin, gout, out=None, stream=None):
     z, zp = _host_f32(z, "z")
     if out is None:
         out = np.empty((go.ny, go.nx), dtype=np.float32)
-    out, op = _host_f32(out, "out")
+    out, op = _host_out_f32(out, go)
     _check(lib().interp_spline_host(zp, gi, op, go, _stream(stream)), "interp_spline_host")
     return out
 
@@ -263,6 +349,13 @@ def interp_bilinear_host_async(z, gin, gout, out, stream=None):
     """Enqueue only (include/bathy.h): `out` is defined after the caller synchronises `stream`."""
     _check(lib().interp_bilinear_host_async(_pinned_f32(z, "z"), _geom(gin), _pinned_f32(out, "out"), _geom(gout),
                                             _stream(stream)), "interp_bilinear_host_async")
+    return out
+
+
+def interp_catmull_rom_host_async(z, gin, gout, out, stream=None):
+    """Enqueue only (include/bathy.h): `out` is defined after the caller synchronises `stream`."""
+    _check(lib().interp_catmull_rom_host_async(_pinned_f32(z, "z"), _geom(gin), _pinned_f32(out, "out"), _geom(gout),
+                                               _stream(stream)), "interp_catmull_rom_host_async")
     return out
 
 
@@ -292,7 +385,7 @@ def krige_host(x, y, z, gout, model, range_, sill, nugget, k, cell_size: float =
     z, zp = _host_f32(z, "z")
     if out is None:
         out = np.empty((go.ny, go.nx), dtype=np.float32)
-    out, op = _host_f32(out, "out")
+    out, op = _host_out_f32(out, go)
     failed = C.c_int64(0)
     vg = Variogram(int(model), float(range_), float(sill), float(nugget))
     n = x.numel() if isinstance(x, torch.Tensor) else x.shape[0]

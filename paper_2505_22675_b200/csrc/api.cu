@@ -10,10 +10,13 @@ int launch_catmull_rom(const float*, const grid_geom_t&, float*, const grid_geom
 size_t spline_workspace_bytes(const grid_geom_t&, const grid_geom_t&);
 int launch_spline(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t, int path);
 int build_index(const float*, const float*, const float*, int64_t, float, cudaStream_t, krige_index**);
+int create_index(float, float, float, float, float, int64_t, cudaStream_t, krige_index**);
+int append_index(krige_index*, const float*, const float*, const float*, int64_t, float*, cudaStream_t);
+int index_header(const krige_index*, IndexHeader*);
 void free_index(krige_index*);
 void free_index_async(krige_index*, cudaStream_t);
-int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, int, float*, int32_t*, int64_t*,
-                   cudaStream_t);
+int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, int, float*, float*, int32_t*, int64_t*,
+                   int64_t*, cudaStream_t);
 
 static std::atomic<int64_t> g_launches{0};
 static std::atomic<int> g_spline_path{0};
@@ -21,7 +24,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 static int check_variogram(const variogram_t& v)
 {
-    if (v.model != BATHY_VGM_EXPONENTIAL && v.model != BATHY_VGM_SPHERICAL) return BATHY_ERR_VARIOGRAM;
+    if (v.model != BATHY_VGM_EXPONENTIAL && v.model != BATHY_VGM_SPHERICAL && v.model != BATHY_VGM_GAUSSIAN) return BATHY_ERR_VARIOGRAM;
     if (!isfinite(v.range) || !isfinite(v.sill) || !isfinite(v.nugget)) return BATHY_ERR_VARIOGRAM;
     if (!(v.range > 0.0f) || !(v.sill > 0.0f) || v.nugget < 0.0f || v.nugget > v.sill) return BATHY_ERR_VARIOGRAM;
     return BATHY_OK;
@@ -101,8 +104,45 @@ BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram
     rc = check_variogram(vg);
     if (rc) return rc;
     if (k < 1 || k > BATHY_MAX_K || (int64_t)k > idx->n) return BATHY_ERR_K;
-    return launch_predict(idx, out, vg, k, d_zhat, d_nbr_or_null, d_failed_or_null,
+    return launch_predict(idx, out, vg, k, d_zhat, nullptr, d_nbr_or_null, d_failed_or_null, nullptr,
                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variogram_t vg, int32_t k,
+                     float* d_zhat, const krige_outputs_t* outputs_or_null, void* cuda_stream)
+{
+    if (!idx || idx->magic != kIndexMagic) return BATHY_ERR_INDEX;
+    if (!d_zhat) return BATHY_ERR_NULL;
+    int rc = check_out_geom(out);
+    if (rc) return rc;
+    rc = check_variogram(vg);
+    if (rc) return rc;
+    if (k < 1 || k > BATHY_MAX_K || (int64_t)k > idx->n) return BATHY_ERR_K;
+    krige_outputs_t o = {nullptr, nullptr, nullptr, nullptr};
+    if (outputs_or_null) o = *outputs_or_null;
+    return launch_predict(idx, out, vg, k, d_zhat, o.d_var, o.d_nbr, o.d_failed, o.d_illcond,
+                          static_cast<cudaStream_t>(cuda_stream));
+}
+
+BATHY_API int krige_index_create(float xmin, float xmax, float ymin, float ymax, float cell_size, int64_t capacity,
+                       void* cuda_stream, krige_index_t** out_index)
+{
+    if (!out_index) return BATHY_ERR_NULL;
+    *out_index = nullptr;
+    if (capacity < 1 || capacity > 0x7fffffffLL) return BATHY_ERR_SIZE;
+    if (!isfinite(xmin) || !isfinite(xmax) || !isfinite(ymin) || !isfinite(ymax) || !(xmax >= xmin) || !(ymax >= ymin))
+        return BATHY_ERR_GEOMETRY;
+    if (!(cell_size >= 0.0f) || !isfinite(cell_size)) return BATHY_ERR_GEOMETRY;
+    return create_index(xmin, xmax, ymin, ymax, cell_size, capacity, static_cast<cudaStream_t>(cuda_stream), out_index);
+}
+
+BATHY_API int krige_index_append(krige_index_t* idx, const float* d_x, const float* d_y, const float* d_z, int64_t n,
+                       float* d_changed_bbox_or_null, void* cuda_stream)
+{
+    if (!idx || idx->magic != kIndexMagic) return BATHY_ERR_INDEX;
+    if (!d_x || !d_y || !d_z) return BATHY_ERR_NULL;
+    if (n < 1) return BATHY_ERR_SIZE;
+    return append_index(idx, d_x, d_y, d_z, n, d_changed_bbox_or_null, static_cast<cudaStream_t>(cuda_stream));
 }
 
 BATHY_API void krige_free_index(krige_index_t* idx) { free_index(idx); }
@@ -111,11 +151,14 @@ BATHY_API void krige_free_index_async(krige_index_t* idx, void* cuda_stream) { f
 BATHY_API int krige_index_info(const krige_index_t* idx, int64_t* n, float* cell_size, int32_t* ncx, int32_t* ncy)
 {
     if (!idx || idx->magic != kIndexMagic) return BATHY_ERR_INDEX;
-    if (n) *n = idx->n;
-    if (cell_size) *cell_size = idx->cell;
-    if (ncx) *ncx = idx->ncx;
-    if (ncy) *ncy = idx->ncy;
-    return BATHY_OK;
+    IndexHeader h;
+    const int rc = index_header(idx, &h);                  // waits for the build / append to finish
+    if (rc) return rc;
+    if (n) *n = h.n;
+    if (cell_size) *cell_size = h.cell;
+    if (ncx) *ncx = h.ncx;
+    if (ncy) *ncy = h.ncy;
+    return h.status;                                       // BATHY_ERR_GEOMETRY: non-finite soundings
 }
 
 }  // extern "C"
@@ -124,7 +167,9 @@ namespace {
 
 // The host-buffer forms: `wait` = synchronise the stream before returning (the plain forms), else
 // everything (allocations, copies, kernels, releases) is only enqueued on the stream (`*_async`).
-int bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream, bool wait)
+typedef int (*grid_launch_fn)(const float*, const grid_geom_t&, float*, const grid_geom_t&, cudaStream_t);
+
+int gather_host(grid_launch_fn launch, const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream, bool wait)
 {
     if (!h_in || !h_out) return BATHY_ERR_NULL;
     int rc = check_in_geom(in);
@@ -136,7 +181,7 @@ int bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t o
     DevBuf din(s), dout(s);
     if (din.alloc(nin) || dout.alloc(nout)) return BATHY_ERR_CUDA;
     BATHY_CUDA_TRY(cudaMemcpyAsync(din.p, h_in, nin, cudaMemcpyHostToDevice, s));
-    rc = launch_bilinear(static_cast<const float*>(din.p), in, static_cast<float*>(dout.p), out, s);
+    rc = launch(static_cast<const float*>(din.p), in, static_cast<float*>(dout.p), out, s);
     if (rc) return rc;
     BATHY_CUDA_TRY(cudaMemcpyAsync(h_out, dout.p, nout, cudaMemcpyDeviceToHost, s));
     if (wait) BATHY_CUDA_TRY(cudaStreamSynchronize(s));
@@ -186,7 +231,7 @@ int krige_host_impl(const float* h_x, const float* h_y, const float* h_z, int64_
     rc = build_index(static_cast<const float*>(dx.p), static_cast<const float*>(dy.p), static_cast<const float*>(dz.p),
                      n, cell_size, s, &idx);
     if (rc) return rc;
-    rc = launch_predict(idx, out, vg, k, static_cast<float*>(dout.p), nullptr, static_cast<int64_t*>(dfail.p), s);
+    rc = launch_predict(idx, out, vg, k, static_cast<float*>(dout.p), nullptr, nullptr, static_cast<int64_t*>(dfail.p), nullptr, s);
     if (rc == BATHY_OK) {
         cudaError_t e = cudaMemcpyAsync(h_zhat, dout.p, nout, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess && h_failed_or_null)
@@ -203,9 +248,13 @@ int krige_host_impl(const float* h_x, const float* h_y, const float* h_z, int64_
 extern "C" {
 
 BATHY_API int interp_bilinear_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
-{ return bilinear_host(h_in, in, h_out, out, cuda_stream, true); }
+{ return gather_host(launch_bilinear, h_in, in, h_out, out, cuda_stream, true); }
 BATHY_API int interp_bilinear_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
-{ return bilinear_host(h_in, in, h_out, out, cuda_stream, false); }
+{ return gather_host(launch_bilinear, h_in, in, h_out, out, cuda_stream, false); }
+BATHY_API int interp_catmull_rom_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+{ return gather_host(launch_catmull_rom, h_in, in, h_out, out, cuda_stream, true); }
+BATHY_API int interp_catmull_rom_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
+{ return gather_host(launch_catmull_rom, h_in, in, h_out, out, cuda_stream, false); }
 BATHY_API int interp_spline_host(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)
 { return spline_host(h_in, in, h_out, out, cuda_stream, true); }
 BATHY_API int interp_spline_host_async(const float* h_in, grid_geom_t in, float* h_out, grid_geom_t out, void* cuda_stream)

@@ -207,12 +207,13 @@ int launch_bilinear(const float* d_in, const grid_geom_t& in, float* d_out, cons
     const long long fw = footprint_bound(ax, TW), fh = footprint_bound(ay, TH);
     const long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
     if (smem <= 160 * 1024 && (out.ny + TH - 1) / TH <= 65535) {
-        static bool attr_set = false;
-        if (!attr_set) {
+        static DeviceOnce once;
+        const int rc = once_per_device(once, []() -> int {
             BATHY_CUDA_TRY(cudaFuncSetAttribute(bilinear_tiled_kernel<CPT, TH>,
                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-            attr_set = true;
-        }
+            return (int)BATHY_OK;
+        });
+        if (rc) return rc;
         dim3 grid((out.nx + TW - 1) / TW, (out.ny + TH - 1) / TH);
         bilinear_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay);
     } else {

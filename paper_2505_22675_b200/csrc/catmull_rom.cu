@@ -298,12 +298,13 @@ int launch_catmull_rom(const float* d_in, const grid_geom_t& in, float* d_out, c
     const long long fw = footprint_bound(ax, TW) + 2, fh = footprint_bound(ay, TH) + 2;
     const long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
     if (smem <= 160 * 1024 && (out.ny + TH - 1) / TH <= 65535) {
-        static bool attr_set = false;
-        if (!attr_set) {
+        static DeviceOnce once;
+        const int rc = once_per_device(once, []() -> int {
             BATHY_CUDA_TRY(cudaFuncSetAttribute(catmull_rom_tiled_kernel<CPT, TH>,
                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-            attr_set = true;
-        }
+            return (int)BATHY_OK;
+        });
+        if (rc) return rc;
         dim3 grid((out.nx + TW - 1) / TW, (out.ny + TH - 1) / TH);
         catmull_rom_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay);
     } else {

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <math.h>
+#include <atomic>
 #include "../../include/bathy.h"
 
 namespace bathy {
@@ -14,8 +15,24 @@ void count_launch(int n = 1);        // api.cu: backs bathy_launch_count()
 #define BATHY_CUDA_TRY(expr)                         \
     do {                                             \
         cudaError_t e__ = (expr);                    \
-        if (e__ != cudaSuccess) return BATHY_ERR_CUDA; \
+        if (e__ != cudaSuccess) { cudaGetLastError(); return BATHY_ERR_CUDA; } /* (clears the non-sticky error) */ \
     } while (0)
+
+// Runs `f` (a cudaFuncSetAttribute sequence) once per CUDA DEVICE of this process: function attributes
+// are per device, so a process-wide flag would leave the second device of a process without them.
+// Thread-safe; a racing first call runs f twice, which is harmless.
+struct DeviceOnce { std::atomic<unsigned long long> mask{0}; };
+template <class F>
+inline int once_per_device(DeviceOnce& o, F f)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return BATHY_ERR_CUDA;
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (dev < 64 && (o.mask.load(std::memory_order_acquire) & bit)) return BATHY_OK;
+    const int rc = f();
+    if (rc == BATHY_OK && dev < 64) o.mask.fetch_or(bit, std::memory_order_release);
+    return rc;
+}
 
 inline int launch_status() { return cudaGetLastError() == cudaSuccess ? BATHY_OK : BATHY_ERR_CUDA; }
 

@@ -1,16 +1,39 @@
 // krige_index.cuh -- the library-owned sounding index.
+//
+// Everything a kernel needs to know about the cell grid lives in a DEVICE header that the build
+// kernels write and krige_predict reads, so that building (or appending to) an index never has to
+// bring the bounding box back to the host: every call only enqueues work.
 #pragma once
 #include "common.cuh"
 
+namespace bathy {
+
+struct IndexHeader {
+    float   xmin, ymin;         // lower corner of the cell grid
+    float   cell, inv_cell;     // cell edge and its fp32 reciprocal
+    int32_t ncx, ncy;           // cell grid
+    float   step_hint;          // mean spacing sqrt(area / n), seeds the first search radius
+    int32_t status;             // BATHY_OK, or BATHY_ERR_GEOMETRY once a non-finite coordinate was seen
+    int32_t n;                  // soundings in the index
+    float   bb[4];              // xmin, xmax, ymin, ymax of all soundings so far
+    float   changed[4];         // xmin, xmax, ymin, ymax of the soundings of the last append
+    int32_t pad[3];
+};
+
+}  // namespace bathy
+
 struct krige_index {
     uint32_t magic;             // kIndexMagic while alive
-    int64_t  n;                 // soundings
-    float    xmin, ymin;        // lower corner of the bounding box
-    float    cell, inv_cell;    // cell edge and its fp32 reciprocal
-    int32_t  ncx, ncy;          // cell grid
-    float    step_hint;         // mean spacing sqrt(area / n), seeds the first search radius
-    float4*  d_pts;             // [n] cell-sorted (x, y, z, original index as int bits)
-    int32_t* d_cell_start;      // [ncx*ncy + 1] exclusive prefix of the per-cell counts
+    int64_t  n;                 // soundings (host count: the sum of what was appended)
+    int64_t  capacity;          // soundings the point buffers hold
+    int64_t  cells_cap;         // cells the cell arrays hold
+    int      device;            // CUDA device the memory lives on
+    bathy::IndexHeader* d_hdr;  // device header (what the kernels read)
+    cudaStream_t stream;        // stream of the last build / append (krige_free_index waits on it)
+    float4*  d_pts;             // [capacity] cell-sorted (x, y, z, original index as int bits)
+    float4*  d_pts_alt;         // [capacity] second buffer of an appendable index (ping-pong), else NULL
+    int32_t* d_cell_start;      // [cells_cap + 1] exclusive prefix of the per-cell counts
+    int32_t* d_cell_start_alt;  // [cells_cap + 1] second buffer of an appendable index, else NULL
 };
 
 namespace bathy {

@@ -38,11 +38,21 @@ constexpr int kBuckets = 32;                     // key histogram of the per-nod
 constexpr int kCrit = 16;                        // listed candidates of the critical bucket
 constexpr float kPivEps = 1e-6f;                 // smallest accepted Cholesky pivot (sill = 1)
 
+// The cell grid of the index, read from its DEVICE header at kernel start (the host never sees it:
+// krige_build_index only enqueues) and kept in shared memory; r0 / rmax are derived from it there.
+struct GridInfo {
+    float xmin, ymin, inv_cell, cell;
+    int ncx, ncy;
+    float r0;           // first pilot radius
+    float rmax;         // radius that certainly covers every sounding from any node of this call
+    int bad;            // the index is unusable (non-finite soundings, or fewer than k of them): every node fails
+};
+
 struct PredictParams {
     const float4* pts;
     const int32_t* cell_start;
-    float xmin, ymin, inv_cell, cell;
-    int ncx, ncy;
+    const IndexHeader* hdr;
+    float r0_factor;    // first pilot radius / mean sounding spacing: the radius that holds ~1.5 k soundings
     int nx, ny;
     float x0, y0, dx, dy;
     int k;
@@ -50,11 +60,12 @@ struct PredictParams {
     float lc;           // log2(cpn)                                   (exponential)
     float c05, c15;     // 0.5 cpn, -1.5 cpn                           (spherical)
     float s_coord;      // coordinate scale of the solve: log2(e)/a (exponential), 1/a (spherical)
-    float r0;           // first pilot radius
-    float rmax;         // radius that certainly covers every sounding from any node of this call
+    float sill;         // kriging variance is reported in the units of sill
     float* zhat;
+    float* var;         // kriging variance (or NULL)
     int32_t* nbr;
     unsigned long long* failed;
+    unsigned long long* illcond;
     int nbx, nby;       // blocks per row / column of blocks
     int chain;          // consecutive blocks walked by one warp
     long long n_blocks;
@@ -120,19 +131,20 @@ __device__ __forceinline__ float ex2_approx(float v)
 // the scan compacts the kept ones: store(slot, pt) is called with consecutive slots.  Returns the
 // number kept (it may exceed `cap`, in which case the stores beyond cap were skipped).
 template <class Keep, class Store>
-__device__ __forceinline__ int scan_cells(const PredictParams& p, int lane, float xlo, float xhi, float ylo, float yhi,
+__device__ __forceinline__ int scan_cells(const PredictParams& p, const GridInfo& gi, int lane, float xlo, float xhi, float ylo, float yhi,
                                           int cap, Keep keep_fn, Store store_fn)
 {
-    const float slack = 2e-3f * p.cell;                    // cell_of() rounding slack
-    const int cx0 = cell_of(xlo - slack, p.xmin, p.inv_cell, p.ncx), cx1 = cell_of(xhi + slack, p.xmin, p.inv_cell, p.ncx);
-    const int cy0 = cell_of(ylo - slack, p.ymin, p.inv_cell, p.ncy), cy1 = cell_of(yhi + slack, p.ymin, p.inv_cell, p.ncy);
+    const float slack = 2e-3f * gi.cell;                   // cell_of() rounding slack
+    const int ncx = gi.ncx;
+    const int cx0 = cell_of(xlo - slack, gi.xmin, gi.inv_cell, ncx), cx1 = cell_of(xhi + slack, gi.xmin, gi.inv_cell, ncx);
+    const int cy0 = cell_of(ylo - slack, gi.ymin, gi.inv_cell, gi.ncy), cy1 = cell_of(yhi + slack, gi.ymin, gi.inv_cell, gi.ncy);
     int n = 0;
     for (int cyb = cy0; cyb <= cy1; cyb += 32) {
         const int cy = cyb + lane;
         int seg_s = 0, seg_e = 0;
         if (cy <= cy1) {
-            seg_s = __ldg(p.cell_start + (size_t)cy * p.ncx + cx0);
-            seg_e = __ldg(p.cell_start + (size_t)cy * p.ncx + cx1 + 1);
+            seg_s = __ldg(p.cell_start + (size_t)cy * ncx + cx0);
+            seg_e = __ldg(p.cell_start + (size_t)cy * ncx + cx1 + 1);
         }
         const int rows = min(32, cy1 - cyb + 1);
         for (int rr = 0; rr < rows; ++rr) {
@@ -159,7 +171,7 @@ __device__ __forceinline__ int scan_cells(const PredictParams& p, int lane, floa
 // `r` is the radius to try first and returns the radius that worked.  Returns a negative value for
 // degenerate input (more than CAP soundings at one distance).
 template <int K, int G>
-__device__ __forceinline__ float pilot(const PredictParams& p, WarpSmem<K, G>& ws, int lane, float cx, float cy, float& r)
+__device__ __forceinline__ float pilot(const PredictParams& p, const GridInfo& gi, WarpSmem<K, G>& ws, int lane, float cx, float cy, float& r)
 {
     using S = Shape<K, G>;
     const int k = p.k;
@@ -170,13 +182,13 @@ __device__ __forceinline__ float pilot(const PredictParams& p, WarpSmem<K, G>& w
     bool found = false;
     for (int it = 0; it < 96; ++it) {
         key_hi = __float_as_uint(fminf(r * r * 1.00001f, 3.0e38f));
-        n = scan_cells(p, lane, cx - r, cx + r, cy - r, cy + r, S::CAP,
+        n = scan_cells(p, gi, lane, cx - r, cx + r, cy - r, cy + r, S::CAP,
                        [&](const float4& pt) { return __float_as_uint(knn_key(cx, cy, pt.x, pt.y)) <= key_hi; },
                        [&](int slot, const float4& pt) { keys[slot] = __float_as_uint(knn_key(cx, cy, pt.x, pt.y)); });
         if (n < k) {
-            if (r >= p.rmax) break;                        // cannot happen for k <= n
+            if (r >= gi.rmax) break;                       // cannot happen for k <= n
             r_low = r;
-            r = isinf(r_high) ? fminf(r * 1.5f, p.rmax) : 0.5f * (r_low + r_high);
+            r = isinf(r_high) ? fminf(r * 1.5f, gi.rmax) : 0.5f * (r_low + r_high);
         } else if (n > S::CAP) {
             r_high = r;
             r = 0.5f * (r_low + r_high);
@@ -339,7 +351,7 @@ __device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSme
 
 // Two covariances at once, normalised to sill = 1, from squared distances in SCALED coordinates (h2 > 0):
 // exponential C = cpn exp(-h/a) = 2^(log2 cpn - h log2(e)/a) (no factor 3);
-// spherical   C = cpn (1 - 1.5 q + 0.5 q^3), q = min(h/a, 1).  h2 == 0 gives NaN (0 * inf): two
+// spherical   C = cpn (1 - 1.5 q + 0.5 q^3), q = min(h/a, 1);  Gaussian C = cpn exp(-(h/a)^2) (NEXT-4).  h2 == 0 gives NaN (0 * inf): two
 // soundings at one place make the system singular and the node fails (reading K-dup).
 // The distance and polynomial arithmetic is packed fp32x2; the two rsqrt and the two ex2 go to the
 // MUFU pipe one by one.
@@ -349,7 +361,13 @@ __device__ __forceinline__ u64 cov2_scaled(u64 h2, const PredictParams& p)
     const u64 rs2 = pack2(rsqrt_approx(lo_of(h2)), rsqrt_approx(hi_of(h2)));
     const u64 q2 = fmul2(h2, rs2);                         // scaled distances
     if (MODEL == BATHY_VGM_EXPONENTIAL) {
-        return pack2(ex2_approx(p.lc - lo_of(q2)), ex2_approx(p.lc - hi_of(q2)));
+        const u64 a2 = ffma2(q2, pack2(-1.0f, -1.0f), pack2(p.lc, p.lc));
+        return pack2(ex2_approx(lo_of(a2)), ex2_approx(hi_of(a2)));
+    } else if (MODEL == BATHY_VGM_GAUSSIAN) {
+        // C = cpn exp(-(h/a)^2) = 2^(log2 cpn - q^2), coordinates pre-scaled by sqrt(log2 e)/a; q = h2 rsqrt(h2)
+        // rather than h2 itself so that h2 == 0 (duplicate soundings) still gives NaN
+        const u64 a2 = ffma2(fmul2(q2, pack2(-1.0f, -1.0f)), q2, pack2(p.lc, p.lc));
+        return pack2(ex2_approx(lo_of(a2)), ex2_approx(hi_of(a2)));
     } else {
         float qa, qb;
         asm("min.NaN.f32 %0, %1, %2;" : "=f"(qa) : "f"(lo_of(q2)), "f"(1.0f));   // NaN (h2 == 0) survives
@@ -423,6 +441,7 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
     float pmin = 1.0f;               // smallest pivot (a NaN pivot poisons every later column and the estimate)
     u64 dots_c = pack2(0.0f, 0.0f);  // (y_c.y_z, y_c.y_1)
     u64 dots_1 = pack2(0.0f, 0.0f);  // (y_1.y_z, y_1.y_1)
+    float dcc = 0.0f;                // y_c.y_c (kriging variance)
     if (g == 0) ws.rhs[1][nd] = make_float4(lo_of(yz1[0]), hi_of(yz1[0]), yc[0], lo_of(A2[0][0]));
     __syncwarp();
     ulonglong2 P = *reinterpret_cast<const ulonglong2*>(&ws.rhs[1][nd]);
@@ -436,6 +455,7 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
         const float ycj = lo_of(P.y) * inv, y1j = hi_of(yj);
         dots_c = ffma2(pack2(ycj, ycj), yj, dots_c);
         dots_1 = ffma2(pack2(y1j, y1j), yj, dots_1);
+        dcc = fmaf(ycj, ycj, dcc);
         float nLr[R];
 #pragma unroll
         for (int t = tj; t < R; ++t) {
@@ -479,11 +499,16 @@ __device__ __forceinline__ void solve_batch(const PredictParams& p, WarpSmem<K, 
         const float dcz = lo_of(dots_c), d1c = hi_of(dots_c), d1z = lo_of(dots_1), d11 = hi_of(dots_1);
         const float mu = (d1c - 1.0f) / d11;
         float est = zref + (dcz - mu * d1z);
+        // kriging variance (sill = 1): 1 - c0^T C^-1 c0 + mu (1^T C^-1 c0 - 1) = 1 - y_c.y_c + mu^2 (y_1.y_1)
+        float var = p.sill * ((1.0f - dcc) + mu * mu * d11);
         if (!(pmin > kPivEps) || !(est == est)) {
-            est = __int_as_float(0x7fc00000);
+            est = var = __int_as_float(0x7fc00000);
             if (p.failed) atomicAdd(p.failed, 1ull);
+        } else if (p.illcond && pmin < BATHY_ILLCOND_PIVOT) {
+            atomicAdd(p.illcond, 1ull);
         }
         p.zhat[node] = est;
+        if (p.var) p.var[node] = var;
     }
 }
 
@@ -500,7 +525,37 @@ krige_predict_kernel(const PredictParams p)
     const long long b1 = min(b0 + (long long)p.chain, p.n_blocks);
     const int k = p.k;
     const float qnan = __int_as_float(0x7fc00000);
-    float rho = p.r0;                                      // pilot radius to try first
+    __shared__ GridInfo gi;
+    if (threadIdx.x == 0) {
+        const IndexHeader h = *p.hdr;
+        gi.xmin = h.xmin; gi.ymin = h.ymin; gi.inv_cell = h.inv_cell; gi.cell = h.cell; gi.ncx = h.ncx; gi.ncy = h.ncy;
+        // farthest any node of this call can be from any sounding: covers the union of both extents
+        const double bx1 = (double)h.xmin + (double)h.ncx * h.cell, by1 = (double)h.ymin + (double)h.ncy * h.cell;
+        const double bx0 = fmin((double)h.xmin, (double)h.bb[0]), by0 = fmin((double)h.ymin, (double)h.bb[2]);
+        const double gx1 = (double)p.x0 + (double)(p.nx - 1) * p.dx, gy1 = (double)p.y0 + (double)(p.ny - 1) * p.dy;
+        const double lox = fmin(bx0, fmin((double)p.x0, gx1)), hix = fmax(fmax(bx1, (double)h.bb[1]), fmax((double)p.x0, gx1));
+        const double loy = fmin(by0, fmin((double)p.y0, gy1)), hiy = fmax(fmax(by1, (double)h.bb[3]), fmax((double)p.y0, gy1));
+        float rmax = (float)(1.01 * ((hix - lox) + (hiy - loy)) + 1.0);
+        float r0 = h.step_hint * p.r0_factor;              // the radius that holds ~1.5 k soundings at the mean density
+        if (!(r0 > 0.0f) || !isfinite(r0)) r0 = rmax;
+        if (r0 > rmax) r0 = rmax;
+        gi.r0 = r0; gi.rmax = rmax;
+        gi.bad = (h.status != BATHY_OK) || (h.n < k) || !isfinite(rmax);
+    }
+    __syncthreads();
+    if (gi.bad) {                                          // CTA-uniform: every node of the call fails
+        for (long long blk = b0; blk < b1; ++blk) {
+            const int bj = (int)(blk % p.nbx), bi = (int)(blk / p.nbx);
+            const int J = bj * BW + (lane & (BW - 1)), I = bi * BH + (lane / BW);
+            if (J < p.nx && I < p.ny) {
+                p.zhat[(long long)I * p.nx + J] = qnan;
+                if (p.var) p.var[(long long)I * p.nx + J] = qnan;
+                if (p.failed) atomicAdd(p.failed, 1ull);
+            }
+        }
+        return;
+    }
+    float rho = gi.r0;                                     // pilot radius to try first
 
 #pragma unroll 1
     for (int it = 0; it < p.chain; ++it) {
@@ -536,7 +591,7 @@ krige_predict_kernel(const PredictParams p)
             const float dmax = sqrtf(ex * ex + ey * ey) * 1.00001f;
 
             __syncwarp();
-            const float T = pilot<K, G>(p, ws, lane, cx, cy, rho);
+            const float T = pilot<K, G>(p, gi, ws, lane, cx, cy, rho);
             bool group_ok = T >= 0.0f;
             int n_c = 0;
             float sT = 0.0f;
@@ -545,7 +600,7 @@ krige_predict_kernel(const PredictParams p)
                 rho = sT * 1.1f + slack;
                 const float Rb = (sT + dmax) * 1.0001f + slack;
                 const float Rb2 = Rb * Rb;
-                n_c = scan_cells(p, lane, cx - ex - Rb, cx + ex + Rb, cy - ey - Rb, cy + ey + Rb, S::CAP,
+                n_c = scan_cells(p, gi, lane, cx - ex - Rb, cx + ex + Rb, cy - ey - Rb, cy + ey + Rb, S::CAP,
                                  [&](const float4& pt) {
                                      const float ax = fmaxf(fabsf(pt.x - cx) - ex, 0.0f), ay = fmaxf(fabsf(pt.y - cy) - ey, 0.0f);
                                      return fmaf(ax, ax, ay * ay) <= Rb2;
@@ -566,7 +621,7 @@ krige_predict_kernel(const PredictParams p)
                 }
                 __syncwarp();
             } else {
-                rho = p.r0;
+                rho = gi.r0;
             }
             bool lane_ok = false;
             if (group_ok) {
@@ -580,6 +635,7 @@ krige_predict_kernel(const PredictParams p)
             }
             if (in_group && !lane_ok) {                    // degenerate input: the node fails
                 p.zhat[node] = qnan;
+                if (p.var) p.var[node] = qnan;
                 if (p.failed) atomicAdd(p.failed, 1ull);
             }
             __syncwarp();
@@ -634,18 +690,23 @@ int launch_shape(const PredictParams& p, int model, cudaStream_t stream)
     const long long ctas = (warps + kWarpsPerCta - 1) / kWarpsPerCta;
     if (ctas > 0x7fffffffLL) return BATHY_ERR_SIZE;
     const size_t smem = sizeof(WarpSmem<K, G>) * kWarpsPerCta;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce once;
+    const int rc = once_per_device(once, [smem]() -> int {
         BATHY_CUDA_TRY(cudaFuncSetAttribute(krige_predict_kernel<K, G, BATHY_VGM_EXPONENTIAL>,
                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         BATHY_CUDA_TRY(cudaFuncSetAttribute(krige_predict_kernel<K, G, BATHY_VGM_SPHERICAL>,
                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+        BATHY_CUDA_TRY(cudaFuncSetAttribute(krige_predict_kernel<K, G, BATHY_VGM_GAUSSIAN>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        return (int)BATHY_OK;
+    });
+    if (rc) return rc;
     if (model == BATHY_VGM_EXPONENTIAL)
         krige_predict_kernel<K, G, BATHY_VGM_EXPONENTIAL><<<(unsigned)ctas, kWarpsPerCta * 32, smem, stream>>>(p);
-    else
+    else if (model == BATHY_VGM_SPHERICAL)
         krige_predict_kernel<K, G, BATHY_VGM_SPHERICAL><<<(unsigned)ctas, kWarpsPerCta * 32, smem, stream>>>(p);
+    else
+        krige_predict_kernel<K, G, BATHY_VGM_GAUSSIAN><<<(unsigned)ctas, kWarpsPerCta * 32, smem, stream>>>(p);
     count_launch();
     return launch_status();
 }
@@ -653,13 +714,12 @@ int launch_shape(const PredictParams& p, int model, cudaStream_t stream)
 }  // namespace
 
 int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogram_t& vg, int k,
-                   float* d_zhat, int32_t* d_nbr, int64_t* d_failed, cudaStream_t stream)
+                   float* d_zhat, float* d_var, int32_t* d_nbr, int64_t* d_failed, int64_t* d_illcond, cudaStream_t stream)
 {
     PredictParams p;
     p.pts = idx->d_pts;
     p.cell_start = idx->d_cell_start;
-    p.xmin = idx->xmin; p.ymin = idx->ymin; p.inv_cell = idx->inv_cell; p.cell = idx->cell;
-    p.ncx = idx->ncx; p.ncy = idx->ncy;
+    p.hdr = idx->d_hdr;
     p.nx = out.nx; p.ny = out.ny; p.x0 = out.x0; p.y0 = out.y0; p.dx = out.dx; p.dy = out.dy;
     p.k = k;
     const double cpn = ((double)vg.sill - (double)vg.nugget) / (double)vg.sill;
@@ -668,22 +728,15 @@ int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogr
     p.c05 = (float)(0.5 * cpn);
     p.c15 = (float)(-1.5 * cpn);
     p.s_coord = (vg.model == BATHY_VGM_EXPONENTIAL) ? (float)(1.4426950408889634 / (double)vg.range)
+              : (vg.model == BATHY_VGM_GAUSSIAN)    ? (float)(sqrt(1.4426950408889634) / (double)vg.range)
                                                     : (float)(1.0 / (double)vg.range);
-    // first pilot radius: the radius that holds ~1.5 k soundings at the mean density
-    p.r0 = (float)((double)idx->step_hint * sqrt(1.5 * (double)k / 3.141592653589793));
-    {
-        // farthest any node of this call can be from any sounding: covers the union of both extents
-        const double bx1 = (double)idx->xmin + (double)idx->ncx * idx->cell, by1 = (double)idx->ymin + (double)idx->ncy * idx->cell;
-        const double gx1 = (double)out.x0 + (double)(out.nx - 1) * out.dx, gy1 = (double)out.y0 + (double)(out.ny - 1) * out.dy;
-        const double lox = fmin((double)idx->xmin, fmin((double)out.x0, gx1)), hix = fmax(bx1, fmax((double)out.x0, gx1));
-        const double loy = fmin((double)idx->ymin, fmin((double)out.y0, gy1)), hiy = fmax(by1, fmax((double)out.y0, gy1));
-        p.rmax = (float)(1.01 * ((hix - lox) + (hiy - loy)) + 1.0);
-        if (!(p.r0 > 0.0f) || !isfinite(p.r0)) p.r0 = p.rmax;
-        if (p.r0 > p.rmax) p.r0 = p.rmax;
-    }
+    p.sill = vg.sill;
+    p.r0_factor = (float)sqrt(1.5 * (double)k / 3.141592653589793);
     p.zhat = d_zhat;
+    p.var = d_var;
     p.nbr = d_nbr;
     p.failed = reinterpret_cast<unsigned long long*>(d_failed);
+    p.illcond = reinterpret_cast<unsigned long long*>(d_illcond);
     p.nbx = (out.nx + BW - 1) / BW;
     p.nby = (out.ny + BH - 1) / BH;
     p.n_blocks = (long long)p.nbx * p.nby;

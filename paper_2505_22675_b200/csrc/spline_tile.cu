@@ -448,12 +448,13 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
 template <class S>
 int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMap& ay, void* d_ws, cudaStream_t stream)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce once;
+    const int rc_attr = once_per_device(once, []() -> int {
         BATHY_CUDA_TRY(cudaFuncSetAttribute(spline_tile_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)S::smem_bytes));
-        attr_set = true;
-    }
+        return (int)BATHY_OK;
+    });
+    if (rc_attr) return rc_attr;
     dim3 grid((ax.n_in - 1 + S::TXI - 1) / S::TXI, (ay.n_in - 1 + S::TYI - 1) / S::TYI);
     float4* colw = static_cast<float4*>(d_ws);
     float4* rowtab = colw + ax.n_out;

@@ -174,8 +174,7 @@ def test_argument_errors():
             b.krige_predict(idx, g, **kw)
         assert e.value.status == status
     idx.free()
-    with pytest.raises(b.BathyError):
-        b.krige_build_index(torch.tensor([0.0, float("nan")], device="cuda"), torch.zeros(2, device="cuda"), torch.zeros(2, device="cuda"))
+    # (non-finite soundings are found on the device: tests/test_gpu_streaming_and_boundary.py)
 
 
 def test_host_form():
@@ -217,13 +216,8 @@ def test_large_coordinates_and_clustered_density():
     got, nbr, failed, _ = _gpu(x, y, z, g, 0, 30.0, sill, 0.05 * sill, 32)
     assert failed == 0 and ref["failed"] == 0
     assert np.array_equal(nbr, ref["nbr"])
-    # in the clump neighbours are centimetres apart: the system is ill-conditioned in fp32, so the depth
-    # bar applies outside it; inside, the estimate must stay within the local data range
-    err = np.abs(got - ref["zhat"])
-    yy, xx = np.meshgrid(np.arange(g.ny) + g.y0, np.arange(g.nx) + g.x0, indexing="ij")
-    outside = (np.abs(xx - 102) > 8) | (np.abs(yy - 102) > 8)
-    assert err[outside].max() <= TOL * depth_range(ref["zhat"])
-    assert err.max() <= 0.5
+    # in the clump neighbours are centimetres apart under a 30 m range; the depth bar holds there too
+    assert max_abs_err(got, ref["zhat"]) <= TOL * depth_range(ref["zhat"])
 
 
 def test_stream_ordered_release_and_rebuild():
