@@ -11,11 +11,16 @@ synthetic input:
     krige_build_index config 4   ~1.0 M multibeam soundings                   (K1)
     krige_predict     config 4   -> 2048^2 nodes, k=32, exponential a=50 m    (K2-K5)
 `value` = output nodes of all three methods per second of device time, inputs resident in HBM.
-`methods` gives nodes/s and the roofline of each method separately (BASELINE.json's metric is
-per method); `roofline` is the one of the kernel that takes most of the step.
+`methods` gives, for EVERY BASELINE.json config (1-5) and method, nodes/s (median and best of >= 20
+separately timed repetitions) and the roofline fraction against both denominators SURVEY.md 8(d)
+names (measured copy bandwidth and nominal 8 TB/s; measured and derived FP32 peak); configs 1-2 fit
+in L2 and are reported warm and cold (L2 flushed before each repetition); config 5 goes through its
+64 tile calls and reports total time, per-tile latency p50/max and the index build separately.
+`roofline` is the one of the kernel that takes most of the step.
 `e2e` is the same step through the C ABI's host-buffer entry points (pinned host memory, the
 host<->device copies inside the timed region).
-Other workloads (`--workload small|config2|config5`) run the same code on the other configs.
+`--workload small|config2|config5` runs the step on other configs; `--no-extras` skips the
+per-config table, the FP32 probe and e2e (short runs under ncu).
 
 N > 1 (torchrun): every rank runs the same step on its own batch (seed + rank): the path shards
 by batch with no data-path collective ("weak").  Time = max over ranks.
@@ -141,10 +146,194 @@ def make_inputs(name: str, rank: int):
 
 # ------------------------------------------------------------------------------------------ our arm
 
+NOMINAL_HBM_GBS = 8000.0                               # the ~8 TB/s north_star names (context denominator)
+
+
+def time_reps(fn, reps, stream, before=None):
+    """Median / best / mean of `reps` separately timed repetitions of fn() (CUDA events on the launching
+    stream); `before()` runs outside the timed bracket of every repetition (L2 flush)."""
+    import torch
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for e0, e1 in evs:
+        if before:
+            before()
+        e0.record(stream)
+        fn()
+        e1.record(stream)
+    torch.cuda.synchronize()
+    ms = sorted(e0.elapsed_time(e1) for e0, e1 in evs)
+    return {"ms_median": ms[len(ms) // 2], "ms_best": ms[0], "ms_mean": float(np.mean(ms)), "reps": reps}
+
+
+def hbm_roof(t, grid_bytes, n_nodes, peaks):
+    sec = t["ms_median"] * 1e-3
+    ach = grid_bytes / sec / 1e9
+    return {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+            "frac_of_nominal_8TBps": ach / NOMINAL_HBM_GBS, "frac_best": grid_bytes / (t["ms_best"] * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "bytes_per_node": grid_bytes / n_nodes}
+
+
+def alu_roof(ms, k, n_nodes, fp32):
+    ach = krige_flops(k) * n_nodes / (ms * 1e-3) / 1e12
+    return {"bound": "alu", "achieved": ach, "peak": fp32["derived"], "unit": "TFLOP/s", "frac": ach / fp32["derived"],
+            "peak_measured": fp32.get("measured"), "frac_of_measured": (ach / fp32["measured"]) if fp32.get("measured") else None,
+            "flop_per_node": krige_flops(k)}
+
+
+def measure_fp32_peak(B, stream, reps=5):
+    """FMA-chain microbenchmark of the library (bathy_probe_fp32): TFLOP/s of scalar FFMA and packed FFMA2."""
+    import torch
+    out = {}
+    for name, packed in (("ffma", False), ("ffma2", True)):
+        best = 0.0
+        B.probe_fp32(packed, 20000, 2)
+        torch.cuda.synchronize()
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            flop = B.probe_fp32(packed, 200000, 2)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            best = max(best, flop / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        out[name] = best
+    return out
+
+
+def grid_methods(B, gw, reps, stream, peaks, flush=None, with_cr=True, z_dev=None):
+    """bilinear / spline / Catmull-Rom of one gridded config: warm (back to back) and, if `flush` is given,
+    cold (L2 flushed before every repetition)."""
+    import torch
+    gi, go = gw.geom_in, gw.geom_out
+    z = z_dev if z_dev is not None else torch.from_numpy(gw.z).cuda()
+    out = torch.empty(go.shape, dtype=torch.float32, device="cuda")
+    ws = torch.empty(B.interp_spline_workspace_bytes(gi, go), dtype=torch.uint8, device="cuda")
+    grid_bytes = 4.0 * (gi.n + go.n)
+    fns = {"bilinear": lambda: B.interp_bilinear(z, gi, go, out=out),
+           "spline": lambda: B.interp_spline(z, gi, go, out=out, workspace=ws)}
+    if with_cr:
+        fns["catmull_rom"] = lambda: B.interp_catmull_rom(z, gi, go, out=out)
+    res = {}
+    for name, fn in fns.items():
+        for _ in range(3):
+            fn()
+        t = time_reps(fn, reps, stream)
+        e = {"nodes": go.n, "nodes_per_s": go.n / (t["ms_median"] * 1e-3), "nodes_per_s_best": go.n / (t["ms_best"] * 1e-3), **t,
+             "roofline": hbm_roof(t, grid_bytes, go.n, peaks)}
+        if flush is not None:
+            tc = time_reps(fn, reps, stream, before=flush)
+            e["cold_l2"] = {"nodes_per_s": go.n / (tc["ms_median"] * 1e-3), **tc, "roofline": hbm_roof(tc, grid_bytes, go.n, peaks)}
+            e["l2"] = "fits in the 126 MB L2: top-level numbers are warm-L2 (back to back), cold_l2 = L2 flushed (512 MB written) before every repetition"
+        else:
+            e["l2"] = "%.0f MB per call exceed the 126 MB L2: no flush needed" % (grid_bytes / 1e6)
+        res[name] = e
+    return res
+
+
+def krige_methods(B, sw, tiles, reps, stream, fp32, flush=None):
+    """krige_build_index and krige_predict of one sounding config (one call, or the tile calls in arrival order)."""
+    import torch
+    from paper_2505_22675_b200 import workloads as W
+    gk = sw.geom_out
+    sx, sy, sz = (torch.from_numpy(a).cuda() for a in (sw.x, sw.y, sw.z))
+    failed = torch.zeros(1, dtype=torch.int64, device="cuda")
+    res = {}
+    hold = []
+
+    def build():
+        hold.append(B.krige_build_index(sx, sy, sz))
+
+    def release():
+        while hold:
+            hold.pop().free_async()
+    for _ in range(3):
+        build(); release()
+    tb = time_reps(lambda: (build(), release()), reps, stream, before=flush)
+    res["krige_build_index"] = {"soundings": int(sw.x.shape[0]), "soundings_per_s": sw.x.shape[0] / (tb["ms_median"] * 1e-3), **tb,
+                                "note": "one-off per survey; not part of nodes/s"}
+    idx = B.krige_build_index(sx, sy, sz)
+    if tiles is None:
+        out = torch.empty(gk.shape, dtype=torch.float32, device="cuda")
+        fn = lambda: B.krige_predict(idx, gk, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=out, failed=failed)
+        n_calls = 1
+    else:
+        tg = [W.tile_geom(gk, i0, j0, ny, nx) for (i0, j0, ny, nx) in tiles]
+        bufs = [torch.empty((t.ny, t.nx), dtype=torch.float32, device="cuda") for t in tg]
+
+        def fn():
+            for t, bf in zip(tg, bufs):
+                B.krige_predict(idx, t, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=bf, failed=failed)
+        n_calls = len(tg)
+    for _ in range(3):
+        fn()
+    t = time_reps(fn, reps, stream, before=flush if tiles is None else None)
+    e = {"nodes": gk.n, "k": sw.k, "launches": n_calls, "nodes_per_s": gk.n / (t["ms_median"] * 1e-3),
+         "nodes_per_s_best": gk.n / (t["ms_best"] * 1e-3), **t, "roofline": alu_roof(t["ms_median"], sw.k, gk.n, fp32)}
+    if tiles is not None:                                   # per-tile latency: events around every tile call of one pass
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(n_calls + 1)]
+        evs[0].record(stream)
+        for i, (tgi, bf) in enumerate(zip(tg, bufs)):
+            B.krige_predict(idx, tgi, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=bf, failed=failed)
+            evs[i + 1].record(stream)
+        torch.cuda.synchronize()
+        lat = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(n_calls))
+        e["tiles"] = {"count": n_calls, "tile_nodes": tg[0].nx * tg[0].ny, "ms_total_first_launch_to_last_completion": float(evs[0].elapsed_time(evs[-1])),
+                      "ms_tile_p50": lat[len(lat) // 2], "ms_tile_max": lat[-1], "ms_tile_min": lat[0]}
+    idx.free()
+    assert int(failed.item()) == 0, "kriging reported failed nodes on a bench workload"
+    res["kriging"] = e
+    return res
+
+
+_WORKLOAD_CACHE = {}
+
+
+def cached_workload(kind, config):
+    """Full-size BASELINE.json workloads are generated once per process (config 5 takes several seconds)."""
+    from paper_2505_22675_b200 import workloads as W
+    key = (kind, config)
+    if key not in _WORKLOAD_CACHE:
+        _WORKLOAD_CACHE[key] = W.grid_config(config) if kind == "grid" else W.sounding_config(config)
+    return _WORKLOAD_CACHE[key]
+
+
+def per_config_table(B, stream, peaks, fp32, reps):
+    """Every BASELINE.json config through the same entry points: {config: {method: numbers}}."""
+    import torch
+    from paper_2505_22675_b200 import workloads as W
+    flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    flush = lambda: flush_buf.fill_(1)
+    table = {}
+    # config 1: kriging (k = 8, spherical) on the valid cells -> 253^2, fill, bilinear + spline on the filled grid
+    w1 = W.grid_config(1)
+    x, y, z = W.grid_to_scattered(w1.z)
+    sill = W.sample_variance(z)
+    sw1 = W.SoundingWorkload(1, x, y, z, w1.geom_out, 8, B.SPHERICAL, 10.0, sill, 0.0)
+    t1 = krige_methods(B, sw1, None, reps, stream, fp32, flush=None)
+    xt, yt, zt = (torch.from_numpy(a).cuda() for a in (x, y, z))
+    idx = B.krige_build_index(xt, yt, zt)
+    fill = B.krige_predict(idx, w1.geom_in, B.SPHERICAL, 10.0, sill, 0.0, 8)
+    idx.free()
+    filled = torch.where(torch.from_numpy(w1.nan_mask).cuda(), fill, torch.from_numpy(w1.z).cuda()).contiguous()
+    t1.update(grid_methods(B, w1, reps, stream, peaks, flush=flush, z_dev=filled))
+    t1["catmull_rom"]["note"] = "on the kriging-filled grid (as bilinear and spline)"
+    table["config1"] = t1
+    # config 2 (L2-resident: warm and cold), config 3 (HBM regime)
+    table["config2"] = grid_methods(B, cached_workload("grid", 2), reps, stream, peaks, flush=flush)
+    table["config3"] = grid_methods(B, cached_workload("grid", 3), reps, stream, peaks)
+    torch.cuda.empty_cache()
+    # config 4 (one call), config 5 (64 tile calls in arrival order)
+    table["config4"] = krige_methods(B, cached_workload("soundings", 4), None, reps, stream, fp32, flush=flush)
+    w5 = cached_workload("soundings", 5)
+    table["config5"] = krige_methods(B, w5, w5.tiles, reps, stream, fp32)
+    del flush_buf
+    return table
+
+
 def run_ours(args):
     import torch
     import paper_2505_22675_b200 as B
     from paper_2505_22675_b200 import workloads as W
+    from paper_2505_22675_b200 import sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -168,7 +357,6 @@ def run_ours(args):
     z_in = torch.from_numpy(gw.z).to(dev)
     out_b = torch.empty(go.shape, dtype=torch.float32, device=dev)
     out_s = torch.empty(go.shape, dtype=torch.float32, device=dev)
-    out_c = torch.empty(go.shape, dtype=torch.float32, device=dev)
     ws = torch.empty(B.interp_spline_workspace_bytes(gi, go), dtype=torch.uint8, device=dev)
     sx, sy, sz = (torch.from_numpy(a).to(dev) for a in (sw.x, sw.y, sw.z))
     out_k = torch.empty(gk.shape, dtype=torch.float32, device=dev)
@@ -219,99 +407,96 @@ def run_ours(args):
 
     seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])        # ms per segment
     total_ms = float(evs[0][0].elapsed_time(evs[-1][4]))
-    from paper_2505_22675_b200 import sharding
     total_ms, ms_bil, ms_spl, ms_idx, ms_krg = sharding.reduce_step_times(
         [total_ms] + seg.mean(axis=0).tolist(), dist, dev)          # max over ranks
     ms_per_step = total_ms / args.steps
+    seg_med = np.median(seg, axis=0).tolist()
+    seg_best = seg.min(axis=0).tolist()
 
-    # ---- NEXT-1: the paper's own Catmull-Rom cubic, timed beside the step (not part of `value`)
-    ec = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    for _ in range(3):
-        B.interp_catmull_rom(z_in, gi, go, out=out_c)
-    barrier()
-    ec[0].record(stream)
-    for _ in range(args.steps):
-        B.interp_catmull_rom(z_in, gi, go, out=out_c)
-    ec[1].record(stream)
-    barrier()
-    ms_cr = sharding.reduce_step_times([ec[0].elapsed_time(ec[1]) / args.steps], dist, dev)[0]
+    peaks = load_peaks()
+    fp32 = {"derived": SMS * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12, "measured": None}
+    table, probe = None, None
+    e2e = None
+    if args.extras:
+        # ---- measured FP32 peak (the library's FMA-chain probe), rank 0 does the reporting but every rank runs it
+        probe = measure_fp32_peak(B, stream)
+        fp32["measured"] = max(probe.values())
 
-    # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the timed region)
-    hz = torch.from_numpy(gw.z).pin_memory()
-    hob = torch.empty(go.shape, dtype=torch.float32).pin_memory()
-    hos = torch.empty(go.shape, dtype=torch.float32).pin_memory()
-    hx, hy, hzz = (torch.from_numpy(a).pin_memory() for a in (sw.x, sw.y, sw.z))
-    hok = torch.empty(gk.shape, dtype=torch.float32).pin_memory()
+        # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the timed region)
+        hz = torch.from_numpy(gw.z).pin_memory()
+        hob = torch.empty(go.shape, dtype=torch.float32).pin_memory()
+        hos = torch.empty(go.shape, dtype=torch.float32).pin_memory()
+        hx, hy, hzz = (torch.from_numpy(a).pin_memory() for a in (sw.x, sw.y, sw.z))
+        hok = torch.empty(gk.shape, dtype=torch.float32).pin_memory()
+        hfail = torch.zeros(1, dtype=torch.int64).pin_memory()
+        # the three methods of the step are enqueued on three streams through the `*_host_async` entry points
+        # (include/bathy.h): the copies of one overlap the kernels and the opposite-direction copies of the
+        # others; the host then waits for all three and reads the results.  The two grid methods go on
+        # high-priority streams: their short kernels must not queue behind the kriging kernel, whose CTAs
+        # fill every SM, because their 268 MB results are what keeps the link busy.
+        st_b, st_s = (torch.cuda.Stream(device=dev, priority=-1) for _ in range(2))
+        st_k = torch.cuda.Stream(device=dev)
 
-    # the three methods of the step are enqueued on three streams through the `*_host_async` entry
-    # points (include/bathy.h): the copies of one overlap the kernels and the opposite-direction copies
-    # of the others; the host then waits for all three and reads the results
-    hfail = torch.zeros(1, dtype=torch.int64).pin_memory()
-    # (kriging is enqueued first -- its one host wait, for the bounding box, must not sit behind the grid
-    # methods' copies -- and the two grid methods go on high-priority streams: their short kernels must
-    # not queue behind the 6 ms kriging kernel, whose CTAs fill every SM, because their 268 MB results are
-    # what keeps the link busy.  Measured: 12.0 ms per step; kriging first without priorities 16.4 ms,
-    # kriging last 17.7 ms, the three synchronous calls in sequence 18.7 ms)
-    st_b, st_s = (torch.cuda.Stream(device=dev, priority=-1) for _ in range(2))
-    st_k = torch.cuda.Stream(device=dev)
+        def e2e_step():
+            B.interp_bilinear_host_async(hz, gi, go, out=hob, stream=st_b.cuda_stream)
+            B.interp_spline_host_async(hz, gi, go, out=hos, stream=st_s.cuda_stream)
+            B.krige_host_async(hx, hy, hzz, gk, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=hok, failed=hfail,
+                               stream=st_k.cuda_stream)
+            st_b.synchronize(); st_s.synchronize(); st_k.synchronize()
+            return float(hok[0, 0]) + float(hob[0, 0]) + float(hos[0, 0]) + int(hfail[0])      # the host reads the result
 
-    def e2e_step():
-        B.krige_host_async(hx, hy, hzz, gk, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=hok, failed=hfail,
-                           stream=st_k.cuda_stream)
-        B.interp_bilinear_host_async(hz, gi, go, out=hob, stream=st_b.cuda_stream)
-        B.interp_spline_host_async(hz, gi, go, out=hos, stream=st_s.cuda_stream)
-        st_b.synchronize(); st_s.synchronize(); st_k.synchronize()
-        return float(hok[0, 0]) + float(hob[0, 0]) + float(hos[0, 0]) + int(hfail[0])      # the host reads the result
-
-    e2e_steps = max(2, min(args.steps, 10))
-    e2e_step()
-    barrier()
-    te0 = time.perf_counter()
-    for _ in range(e2e_steps):
+        e2e_steps = max(2, min(args.steps, 10))
         e2e_step()
-    barrier()
-    e2e_ms = (time.perf_counter() - te0) * 1e3 / e2e_steps
-    e2e_ms = sharding.reduce_step_times([e2e_ms], dist, dev)[0]
-    h2d = 2 * gi.n * 4 + 3 * sw.x.shape[0] * 4
-    d2h = 2 * n_grid * 4 + n_krige * 4 + 8
+        barrier()
+        te0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        barrier()
+        e2e_ms = (time.perf_counter() - te0) * 1e3 / e2e_steps
+        e2e_ms = sharding.reduce_step_times([e2e_ms], dist, dev)[0]
+        e2e = {"value": world * nodes_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+               "h2d_bytes_per_step": 2 * gi.n * 4 + 3 * sw.x.shape[0] * 4, "d2h_bytes_per_step": 2 * n_grid * 4 + n_krige * 4 + 8,
+               "steps": e2e_steps,
+               "api": "interp_bilinear_host_async + interp_spline_host_async + krige_host_async on three streams, then stream synchronize (pinned host buffers); no call blocks the host"}
+        del hz, hob, hos, hx, hy, hzz, hok
 
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
-    peaks = load_peaks()
-    fp32_peak = SMS * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12     # TFLOP/s at the max SM clock
+    if args.extras and world == 1:
+        del z_in, out_b, out_s, out_k, ws
+        torch.cuda.empty_cache()
+        table = per_config_table(B, stream, peaks, fp32, args.reps)
+
     grid_bytes = 4.0 * (gi.n + n_grid)                  # compulsory: input read once, output written once
-    kf = krige_flops(sw.k)
-    meth = {
-        "bilinear": {"nodes_per_s": n_grid / (ms_bil * 1e-3), "ms": ms_bil, "launches": 1,
-                     "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_bil * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
-                                  "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid}},
-        "spline": {"nodes_per_s": n_grid / (ms_spl * 1e-3), "ms": ms_spl,
-                   "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_spl * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
-                                "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid,
-                                "note": "whole call (all its kernels) against the compulsory bytes of the method"}},
-        "catmull_rom": {"nodes_per_s": n_grid / (ms_cr * 1e-3), "ms": ms_cr, "launches": 1, "in_step": False,
-                        "roofline": {"bound": "hbm", "achieved": grid_bytes / (ms_cr * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
-                                     "unit": "GB/s", "bytes_per_node": grid_bytes / n_grid,
-                                     "note": "NEXT-1 (paper's own cubic, PAPER.md:L136-L144); timed beside the step, not in `value`"}},
-        "krige_build_index": {"soundings_per_s": sw.x.shape[0] / (ms_idx * 1e-3), "ms": ms_idx},
-        "kriging": {"nodes_per_s": n_krige / (ms_krg * 1e-3), "ms": ms_krg, "k": sw.k, "launches": len(tiles),
-                    "ms_per_launch": ms_krg / len(tiles),
-                    "roofline": {"bound": "alu", "achieved": kf * n_krige / (ms_krg * 1e-3) / 1e12, "peak": fp32_peak,
-                                 "unit": "TFLOP/s", "flop_per_node": kf}},
+
+    def seg_entry(i, n_nodes):
+        return {"nodes_per_s": n_nodes / (seg_med[i] * 1e-3), "ms": [ms_bil, ms_spl, ms_idx, ms_krg][i], "ms_median": seg_med[i],
+                "ms_best": seg_best[i]}
+    step_methods = {
+        "bilinear": {**seg_entry(0, n_grid), "launches": 1,
+                     "roofline": hbm_roof({"ms_median": ms_bil, "ms_best": seg_best[0]}, grid_bytes, n_grid, peaks)},
+        "spline": {**seg_entry(1, n_grid),
+                   "roofline": hbm_roof({"ms_median": ms_spl, "ms_best": seg_best[1]}, grid_bytes, n_grid, peaks)},
+        "krige_build_index": {"soundings_per_s": sw.x.shape[0] / (ms_idx * 1e-3), "ms": ms_idx, "ms_median": seg_med[2]},
+        "kriging": {**seg_entry(3, n_krige), "k": sw.k, "launches": len(tiles), "ms_per_launch": ms_krg / len(tiles),
+                    "roofline": alu_roof(ms_krg, sw.k, n_krige, fp32)},
     }
-    for m in ("bilinear", "spline", "kriging", "catmull_rom"):
-        r = meth[m]["roofline"]
-        r["frac"] = r["achieved"] / r["peak"]
-    dom = max(("bilinear", "spline", "kriging"), key=lambda m: meth[m]["ms"])
+    dom = max(("bilinear", "spline", "kriging"), key=lambda m: step_methods[m]["ms"])
     kernel_name = {"bilinear": "bilinear_tiled_kernel", "spline": "spline_tables_kernel + spline_tile_kernel",
-                   "kriging": "krige_predict_kernel"}[dom]
-    roof = dict(meth[dom]["roofline"])
+                   "kriging": "krige_predict_kernel<%d>" % (8 if sw.k <= 8 else 16 if sw.k <= 16 else 32 if sw.k <= 32 else 64)}[dom]
+    roof = dict(step_methods[dom]["roofline"])
+    if roof["bound"] == "alu" and fp32["measured"]:
+        # the judged fraction is against the MEASURED FP32 peak; the derived one stays beside it
+        roof.update({"peak": fp32["measured"], "frac": roof["achieved"] / fp32["measured"], "peak_derived": fp32["derived"],
+                     "frac_of_derived": roof["achieved"] / fp32["derived"]})
     roof.update({"kernel": kernel_name, "traffic": None, "peak_source": (
         f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else
-        f"derived: {SMS} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)")})
+        ("measured: bathy_probe_fp32 FMA-chain microbenchmark in this run (best of FFMA / FFMA2); derived beside it: "
+         if fp32["measured"] else "derived: ") +
+        f"{SMS} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz = {fp32['derived']:.1f} TFLOP/s (DESIGN.md)")})
     tr = os.path.join(ROOT, "profiles", "traffic.json")      # DRAM bytes per launch from the committed ncu capture
     if os.path.exists(tr):
         try:
@@ -331,14 +516,16 @@ def run_ours(args):
                           % (grid_bytes / 1e6, 16.0 * sw.x.shape[0] / 1e6, 2 * grid_bytes / 1e6))
                    if grid_bytes > 2.0e8 else "grid data fits L2: warm-L2 numbers for bilinear/spline",
                    "parallelism": f"replicated batches x{world}, no collective"},
-        "methods": meth,
+        "step_methods": step_methods,
+        "methods": table if table is not None else {"step": step_methods},
         "roofline": roof,
-        "e2e": {"value": world * nodes_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-                "api": "interp_bilinear_host_async + interp_spline_host_async + krige_host_async on three streams, then stream synchronize (pinned host buffers)"},
+        "fp32_peak": {"derived_tflops": fp32["derived"], "measured_tflops": fp32["measured"], "probe": probe,
+                      "how": "bathy_probe_fp32: 2 CTAs x 512 threads per SM, 16 independent FMA chains per thread, CUDA events"},
         "gpu_launches": int(n1 - n0),
         "clocks": clocks,
     }
+    if e2e is not None:
+        line["e2e"] = e2e
     if args.cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload, budget_s=args.cpu_budget)
     print(json.dumps(line))
@@ -383,17 +570,44 @@ def extrapolate(sample: dict, n_grid: int, n_krige: int) -> float:
 
 
 def cpu_baseline(name: str, budget_s: float = 20.0) -> dict:
+    """The oracle as it stands on the box's host cores: all cores (the reported baseline) and ONE thread beside it
+    (SURVEY.md 8(d)), bounded samples; plus the k = 64 kriging rate on config 5 when bench.py has it in memory."""
     import oracle
     gw, sw, _ = make_inputs(name, 0)
     cores = oracle.num_threads()
-    # sized for ~10-30 s of CPU work: kriging nodes scale with the thread count
-    kn = int(max(2000, min(sw.geom_out.n, budget_s * 0.6 * cores * 2.0e4 * (32.0 / sw.k) ** 3)))
+    # sized for ~10-20 s of CPU work: kriging nodes scale with the thread count
+    kn = int(max(2000, min(sw.geom_out.n, budget_s * 0.5 * cores * 2.0e4 * (32.0 / sw.k) ** 3)))
     smp = oracle_sample_step(name, gw, sw, krige_nodes=kn, grid_n_in=2048)
-    return {"value": extrapolate(smp, gw.geom_out.n, sw.geom_out.n), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": (f"float64 oracle, OpenMP x{cores}: bilinear+spline on the {min(2048, gw.geom_in.nx)}^2 crop of the input "
-                       f"({smp['bilinear'][1]} nodes each), kriging at {smp['kriging'][1]} evenly spaced nodes with the full "
-                       f"sounding set; per-method rates extrapolated to the step's node mix"),
-            "per_method_nodes_per_s": {m: smp[m][1] / smp[m][0] for m in smp}}
+    oracle.set_num_threads(1)
+    try:
+        kn1 = int(max(500, min(sw.geom_out.n, 4.0 * 2.0e4 * (32.0 / sw.k) ** 3)))
+        smp1 = oracle_sample_step(name, gw, sw, krige_nodes=kn1, grid_n_in=1024)
+    finally:
+        oracle.set_num_threads(cores)
+    out = {"value": extrapolate(smp, gw.geom_out.n, sw.geom_out.n), "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": (f"float64 oracle, OpenMP x{cores}: bilinear+spline on the {min(2048, gw.geom_in.nx)}^2 crop of the input "
+                      f"({smp['bilinear'][1]} nodes each), kriging at {smp['kriging'][1]} evenly spaced nodes with the full "
+                      f"sounding set; per-method rates extrapolated to the step's node mix"),
+           "per_method_nodes_per_s": {m: smp[m][1] / smp[m][0] for m in smp},
+           "one_thread": {"value": extrapolate(smp1, gw.geom_out.n, sw.geom_out.n), "cores": 1,
+                          "per_method_nodes_per_s": {m: smp1[m][1] / smp1[m][0] for m in smp1},
+                          "sample": f"same oracle, 1 thread: 1024^2 crop ({smp1['bilinear'][1]} nodes), kriging at {smp1['kriging'][1]} nodes"}}
+    if ("soundings", 5) in _WORKLOAD_CACHE:
+        w5 = _WORKLOAD_CACHE[("soundings", 5)]
+        v = oracle.vgm(w5.model, w5.range_, w5.sill, w5.nugget)
+        g = w5.geom_out
+        buckets = oracle.Buckets(w5.x, w5.y, 4.0)
+        xq, yq = oracle.node_coords(oracle.geom(g.nx, g.ny, g.x0, g.y0, g.dx, g.dy))
+        rates = {}
+        for thr, nn in ((cores, 12000 * cores), (1, 6000)):
+            oracle.set_num_threads(thr)
+            sel = np.linspace(0, g.n - 1, nn).astype(np.int64)
+            t0 = time.perf_counter()
+            oracle.krige_points(w5.x, w5.y, w5.z, xq.ravel()[sel], yq.ravel()[sel], v, w5.k, buckets, want_nbr=False)
+            rates[f"kriging_k64_config5_x{thr}"] = nn / (time.perf_counter() - t0)
+        oracle.set_num_threads(cores)
+        out["config5_nodes_per_s"] = rates
+    return out
 
 
 def run_reference(args):
@@ -435,6 +649,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="default", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--no-extras", dest="extras", action="store_false",
+                    help="skip the per-config table, the FP32 probe and e2e (short runs under ncu)")
+    ap.add_argument("--reps", type=int, default=20, help="separately timed repetitions per method in the per-config table")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle work in cpu_baseline")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -250,6 +250,15 @@ BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* 
  * their difference (8.2e-7 x depth range per direction). */
 BATHY_API int bathy_set_spline_path(int path);
 
+/* FP32 ALU peak probe ("the builder measures an FMA-chain microbenchmark"): launches one kernel
+ * in which every thread of `ctas_per_sm` (1..4) CTAs of 512 threads per SM runs 16 independent fused multiply-add
+ * chains for `iters` iterations -- scalar FFMA (packed = 0) or packed fp32x2 FFMA2 (packed = 1) -- and writes the
+ * number of floating-point operations the launch retires to *flop_out (host).  The caller times the launch with
+ * CUDA events: flop / time is the measured peak the kriging roofline is reported against.  d_sink: one device
+ * float (never written in practice).  Enqueue only. */
+BATHY_API int bathy_probe_fp32(int32_t packed, int64_t iters, int32_t ctas_per_sm, float* d_sink, double* flop_out,
+                     void* cuda_stream);
+
 /* Static, never NULL. */
 BATHY_API const char* bathy_strerror(int status);
 

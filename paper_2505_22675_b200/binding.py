@@ -26,7 +26,7 @@ SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_byt
            "interp_spline_host", "krige_host", "interp_bilinear_host_async", "interp_spline_host_async",
            "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path",
            "krige_predict_ex", "krige_index_create", "krige_index_append", "interp_catmull_rom_host",
-           "interp_catmull_rom_host_async"]
+           "interp_catmull_rom_host_async", "bathy_probe_fp32"]
 
 
 class GridGeom(C.Structure):
@@ -88,6 +88,7 @@ def lib():
         L.bathy_strerror.restype = C.c_char_p
         L.bathy_launch_count.restype = C.c_int64
         L.bathy_set_spline_path.argtypes = [C.c_int]
+        L.bathy_probe_fp32.argtypes = [C.c_int32, C.c_int64, C.c_int32, vp, C.POINTER(C.c_double), vp]
         _lib = L
     return _lib
 
@@ -117,6 +118,15 @@ def _dev_f32(t: torch.Tensor, name: str) -> torch.Tensor:
 
 def launch_count() -> int:
     return int(lib().bathy_launch_count())
+
+
+def probe_fp32(packed: bool, iters: int, ctas_per_sm: int = 2, stream=None) -> float:
+    """Enqueues the FMA-chain probe (include/bathy.h) and returns the flop it retires; time it with CUDA events."""
+    sink = torch.zeros(1, dtype=torch.float32, device=torch.device("cuda", torch.cuda.current_device()))
+    flop = C.c_double(0.0)
+    _check(lib().bathy_probe_fp32(int(bool(packed)), int(iters), int(ctas_per_sm), sink.data_ptr(), C.byref(flop),
+                                  _stream(stream)), "bathy_probe_fp32")
+    return float(flop.value)
 
 
 def set_spline_path(path: int) -> None:
