@@ -72,6 +72,8 @@ def lib():
         L.oracle_krige_points_var.argtypes = [fp, fp, fp, C.c_int64, C.c_void_p, fp, fp, C.c_int64, vp,
                                               C.c_int, dp, dp, ip]
         L.oracle_krige_points_var.restype = C.c_int64
+        L.oracle_krige_window.argtypes = [fp, gp, C.c_int, C.c_int, C.c_int, vp, dp, C.POINTER(C.c_uint8)]
+        L.oracle_krige_window.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -273,3 +275,20 @@ def krige_grid(x, y, z, g: Geom, v: Vgm, k: int, buckets: Buckets | None = None,
     if r["nbr"] is not None:
         r["nbr"] = r["nbr"].reshape(g.ny, g.nx, k)
     return r
+
+
+def krige_window(z, g: Geom, v: Vgm, half: int = 2, n_max: int | None = None, n_min: int = 3):
+    """NEXT-2: holes (NaN) of a regular grid filled by ordinary kriging from the valid
+    cells of the (2 half + 1)^2 window, bilinear fallback below n_min neighbours.  Returns dict(out float64 [ny, nx],
+    how uint8 [ny, nx], failed)."""
+    z = _f32(z)
+    assert z.shape == (g.ny, g.nx)
+    if n_max is None:
+        n_max = (2 * half + 1) ** 2 - 1
+    out = np.empty((g.ny, g.nx), dtype=np.float64)
+    how = np.empty((g.ny, g.nx), dtype=np.uint8)
+    failed = lib().oracle_krige_window(_p(z, C.c_float), C.byref(g), int(half), int(n_max), int(n_min), C.byref(v),
+                                       _p(out, C.c_double), _p(how, C.c_uint8))
+    if failed < 0:
+        raise ValueError(f"oracle_krige_window: {failed}")
+    return {"out": out, "how": how, "failed": int(failed)}

@@ -579,3 +579,85 @@ int64_t oracle_krige_points_var(const float *x, const float *y, const float *z, 
 {
     return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, k, zhat, nbr_out, NULL, var_out);
 }
+
+/* ================================================================== grid-window kriging (hole filling)
+ * SURVEY.md 8(f) NEXT-2; PAPER.md:L163 ("the implementation in this study uses a 5x5 grid"), L171 and L180
+ * (fallback to bilinear "if enough valid candidate neighbors are not found"), L179 (helper that finds "the
+ * nearest n valid candidate neighbors"), L225-L234 (Grid B: cells removed at random from a regular grid are
+ * interpolated back).  Readings W1-W4 of DESIGN.md:
+ *  W1  a valid (non-NaN) cell is copied; a NaN cell (a hole) at row i, column j is estimated by ordinary kriging
+ *      (K3-K5 above, gamma-form LU) from valid cells of the (2 half + 1)^2 window centred on it, clipped by the grid;
+ *  W2  "nearest n valid": the n_max candidates with the smallest (key, window order), key = fmaf(ddx, ddx, ddy*ddy)
+ *      in fp32 with ddx = (float)dj * dx, ddy = (float)di * dy (fp32 products; dj, di the lattice offsets), window
+ *      order = row-major over the window; neighbours are used in window order;
+ *  W3  fewer than n_min valid candidates -> the bilinear fallback;
+ *  W4  bilinear at a hole = the formula of PAPER.md:L132 on the rectangle spanned by columns j-1, j+1 and rows i-1,
+ *      i+1, which the hole sits in the middle of (t = s = 1/2): the mean of the four diagonal neighbours, NaN if
+ *      one of them is NaN or outside the grid (bilinear has no fallback, L182).
+ * how [ny*nx] (or NULL): 0 = valid cell copied, 1..64 = kriged from that many neighbours, 255 = bilinear fallback.
+ * A singular system gives NaN (counted in the return value). */
+int64_t oracle_krige_window(const float *in, const ora_geom *g, int half, int n_max, int n_min, const ora_vgm *v,
+                            double *out, uint8_t *how)
+{
+    if (!in || !out || g->nx < 2 || g->ny < 2 || half < 1 || half > 3 || n_max < 1 || n_max > 64 || n_min < 1) return -1;
+    if (!(g->dx > 0.0f) || !(g->dy > 0.0f)) return -1;
+    const int nx = g->nx, ny = g->ny, side = 2 * half + 1;
+    int64_t failed = 0;
+    #pragma omp parallel for schedule(dynamic, 8) reduction(+:failed)
+    for (int i = 0; i < ny; ++i) {
+        for (int j = 0; j < nx; ++j) {
+            const size_t at = (size_t)i * nx + j;
+            if (!isnan(in[at])) { out[at] = (double)in[at]; if (how) how[at] = 0; continue; }
+            /* W1: valid cells of the clipped window, in window (row-major) order */
+            int ci[64], cj[64], m = 0;
+            float key[64];
+            for (int a = -half; a <= half; ++a)
+                for (int b = -half; b <= half; ++b) {
+                    int ii = i + a, jj = j + b;
+                    if ((a == 0 && b == 0) || ii < 0 || ii >= ny || jj < 0 || jj >= nx) continue;
+                    if (isnan(in[(size_t)ii * nx + jj])) continue;
+                    volatile float ddx = (float)b * g->dx;
+                    volatile float ddy = (float)a * g->dy;
+                    volatile float pr = ddy * ddy;
+                    ci[m] = ii; cj[m] = jj; key[m] = fmaf(ddx, ddx, pr); ++m;
+                }
+            (void)side;
+            /* W2: keep the n_max nearest by (key, window order) */
+            int keep[64], k = 0;
+            for (int e = 0; e < m; ++e) {
+                int rank = 0;
+                for (int f = 0; f < m; ++f) rank += (key[f] < key[e] || (key[f] == key[e] && f < e));
+                if (rank < n_max) keep[k++] = e;
+            }
+            if (k < n_min) {
+                /* W3 + W4: bilinear on the rectangle of the diagonal neighbours, t = s = 1/2 */
+                double f = NAN;
+                if (i - 1 >= 0 && i + 1 < ny && j - 1 >= 0 && j + 1 < nx) {
+                    double Q11 = in[(size_t)(i - 1) * nx + j - 1], Q21 = in[(size_t)(i - 1) * nx + j + 1];
+                    double Q12 = in[(size_t)(i + 1) * nx + j - 1], Q22 = in[(size_t)(i + 1) * nx + j + 1];
+                    double t = 0.5, s = 0.5;
+                    f = (1.0 - t) * (1.0 - s) * Q11 + t * (1.0 - s) * Q21 + (1.0 - t) * s * Q12 + t * s * Q22;
+                }
+                out[at] = f;
+                if (how) how[at] = 255;
+                continue;
+            }
+            double px[64], py[64], lam[64];
+            for (int e = 0; e < k; ++e) {
+                px[e] = (double)g->x0 + (double)cj[keep[e]] * (double)g->dx;
+                py[e] = (double)g->y0 + (double)ci[keep[e]] * (double)g->dy;
+            }
+            double xq = (double)g->x0 + (double)j * (double)g->dx, yq = (double)g->y0 + (double)i * (double)g->dy;
+            double est = NAN;
+            if (oracle_ok_weights(px, py, k, xq, yq, v, lam, NULL) == 0) {
+                est = 0.0;
+                for (int e = 0; e < k; ++e) est += lam[e] * (double)in[(size_t)ci[keep[e]] * nx + cj[keep[e]]];
+            } else {
+                failed += 1;
+            }
+            out[at] = est;
+            if (how) how[at] = (uint8_t)k;
+        }
+    }
+    return failed;
+}
