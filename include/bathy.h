@@ -197,6 +197,29 @@ BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variog
                      float* d_zhat, const krige_outputs_t* outputs_or_null, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * interp_krige_window -- hole filling on a regular grid by ordinary kriging over a window of grid cells, the form
+ * of kriging the paper measured: "the implementation in this study uses a 5x5 grid"
+ * (PAPER.md:L163); cells removed at random are interpolated back (Grid B, L225-L234).
+ *   - a valid (non-NaN) cell of d_in is copied to d_out;
+ *   - a NaN cell (i, j) is estimated by ordinary kriging (as krige_predict: variogram, ordinary-kriging system,
+ *     z_hat = sum lambda z) from the valid cells of the (2 half + 1)^2 window centred on it, clipped by the grid;
+ *     if more than n_max are valid, the n_max with the smallest (key, window order) are used -- the paper's
+ *     "nearest n valid candidate neighbors" (L179) -- key = fmaf(ddx, ddx, ddy*ddy) in fp32 with ddx = (float)dj * dx,
+ *     ddy = (float)di * dy, window order = row-major over the window;
+ *   - with fewer than n_min valid candidates the cell "falls back to bilinear interpolation" (L171, L180): the
+ *     formula of L132 on the rectangle of its four diagonal neighbours (t = s = 1/2, i.e. their mean); NaN if one
+ *     of them is NaN or outside the grid (bilinear has no fallback, L182).
+ * win.half in [1, 3] (3x3, 5x5 = the paper's, 7x7); win.n_max >= 1 (values above the window size mean "all");
+ * win.n_min >= 1.  d_in [g.ny * g.nx] fp32; d_out the same size, fully overwritten, no overlap with d_in.
+ * d_how_or_null [g.ny * g.nx] uint8: 0 = valid cell copied, 1..48 = kriged from that many neighbours, 255 =
+ * bilinear fallback.  d_failed_or_null as krige_predict.  Enqueue only (scratch comes from the stream's pool). */
+typedef struct {
+    int32_t half, n_max, n_min;
+} krige_window_t;
+BATHY_API int interp_krige_window(const float* d_in, grid_geom_t g, krige_window_t win, variogram_t vg,
+                        float* d_out, uint8_t* d_how_or_null, int64_t* d_failed_or_null, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Streaming index (the paper's real-time onboard goal).
  * krige_index_create makes an EMPTY index over the caller's extent -- the planned survey area
  * [xmin, xmax] x [ymin, ymax]; soundings outside it are legal and are kept in the border cells -- with

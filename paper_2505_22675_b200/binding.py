@@ -26,7 +26,7 @@ SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_byt
            "interp_spline_host", "krige_host", "interp_bilinear_host_async", "interp_spline_host_async",
            "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path",
            "krige_predict_ex", "krige_index_create", "krige_index_append", "interp_catmull_rom_host",
-           "interp_catmull_rom_host_async", "bathy_probe_fp32"]
+           "interp_catmull_rom_host_async", "bathy_probe_fp32", "interp_krige_window"]
 
 
 class GridGeom(C.Structure):
@@ -40,6 +40,10 @@ class Variogram(C.Structure):
 
 class KrigeOutputs(C.Structure):
     _fields_ = [("d_var", C.c_void_p), ("d_nbr", C.c_void_p), ("d_failed", C.c_void_p), ("d_illcond", C.c_void_p)]
+
+
+class KrigeWindow(C.Structure):
+    _fields_ = [("half", C.c_int32), ("n_max", C.c_int32), ("n_min", C.c_int32)]
 
 
 class BathyError(RuntimeError):
@@ -70,6 +74,7 @@ def lib():
         L.krige_predict_ex.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, C.POINTER(KrigeOutputs), vp]
         L.krige_index_create.argtypes = [C.c_float] * 5 + [C.c_int64, vp, C.POINTER(vp)]
         L.krige_index_append.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
+        L.interp_krige_window.argtypes = [vp, GridGeom, KrigeWindow, Variogram, vp, vp, vp, vp]
         L.krige_free_index.argtypes = [vp]
         L.krige_free_index.restype = None
         L.krige_free_index_async.argtypes = [vp, vp]
@@ -268,6 +273,29 @@ def krige_predict(index: KrigeIndex, gout, model: int, range_: float, sill: floa
                "krige_predict_ex")
     res = (out,) + ((nbr,) if want_nbr else ()) + ((var,) if var is not None else ())
     return res if len(res) > 1 else out
+
+
+def interp_krige_window(z: torch.Tensor, geom, model: int, range_: float, sill: float, nugget: float, half: int = 2,
+                        n_max: int | None = None, n_min: int = 3, out: torch.Tensor | None = None, want_how: bool = False,
+                        failed: torch.Tensor | None = None, stream=None):
+    """fills the NaN cells of a regular grid by ordinary kriging
+    over the (2 half + 1)^2 window of grid cells, bilinear fallback below n_min valid neighbours.  Returns out
+    (and how, uint8 [ny, nx], when want_how)."""
+    g = _geom(geom)
+    _dev_f32(z, "z")
+    assert z.numel() == g.nx * g.ny
+    if out is None:
+        out = torch.empty((g.ny, g.nx), dtype=torch.float32, device=z.device)
+    _dev_f32(out, "out")
+    assert out.numel() == g.nx * g.ny and out.data_ptr() != z.data_ptr()
+    how = torch.empty((g.ny, g.nx), dtype=torch.uint8, device=z.device) if want_how else None
+    if n_max is None:
+        n_max = (2 * int(half) + 1) ** 2 - 1
+    vg = Variogram(int(model), float(range_), float(sill), float(nugget))
+    _check(lib().interp_krige_window(z.data_ptr(), g, KrigeWindow(int(half), int(n_max), int(n_min)), vg, out.data_ptr(),
+                                     how.data_ptr() if how is not None else None, _counter(failed, "failed"),
+                                     _stream(stream)), "interp_krige_window")
+    return (out, how) if want_how else out
 
 
 def krige_index_create(xmin: float, xmax: float, ymin: float, ymax: float, capacity: int, cell_size: float = 0.0,

@@ -18,6 +18,9 @@ void free_index_async(krige_index*, cudaStream_t);
 int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, int, float*, float*, int32_t*, int64_t*,
                    int64_t*, cudaStream_t);
 
+int launch_krige_window(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
+                        cudaStream_t);
+
 static std::atomic<int64_t> g_launches{0};
 static std::atomic<int> g_spline_path{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
@@ -122,6 +125,19 @@ BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variog
     if (outputs_or_null) o = *outputs_or_null;
     return launch_predict(idx, out, vg, k, d_zhat, o.d_var, o.d_nbr, o.d_failed, o.d_illcond,
                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+BATHY_API int interp_krige_window(const float* d_in, grid_geom_t g, krige_window_t win, variogram_t vg,
+                        float* d_out, uint8_t* d_how_or_null, int64_t* d_failed_or_null, void* cuda_stream)
+{
+    if (!d_in || !d_out) return BATHY_ERR_NULL;
+    int rc = check_in_geom(g);
+    if (rc) return rc;
+    rc = check_variogram(vg);
+    if (rc) return rc;
+    if (win.half < 1 || win.half > 3 || win.n_max < 1 || win.n_min < 1) return BATHY_ERR_K;
+    return launch_krige_window(d_in, g, win.half, win.n_max, win.n_min, vg, d_out, d_how_or_null, d_failed_or_null,
+                               static_cast<cudaStream_t>(cuda_stream));
 }
 
 BATHY_API int krige_index_create(float xmin, float xmax, float ymin, float ymax, float cell_size, int64_t capacity,
