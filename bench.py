@@ -348,6 +348,67 @@ def per_config_table(B, stream, peaks, fp32, reps):
     return table
 
 
+def run_survey_sharded(args):
+    """--shard survey: ONE config-5 survey split over the ranks -- the soundings of
+    rank 0 are replicated by one NCCL broadcast, every rank builds the same index and predicts the output tiles it
+    owns (round-robin in arrival order); no other collective.  Strong scaling: value = all nodes / slowest rank."""
+    import torch
+    import paper_2505_22675_b200 as B
+    from paper_2505_22675_b200 import workloads as W
+    from paper_2505_22675_b200 import sharding
+
+    world, rank, local = (int(os.environ.get(k, d)) for k, d in (("WORLD_SIZE", "1"), ("RANK", "0"), ("LOCAL_RANK", "0")))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    sw = W.sounding_config(5)                               # same seed on every rank: only rank 0's copy is used
+    gk = sw.geom_out
+    xs = [torch.from_numpy(a).to(dev) if rank == 0 else torch.zeros(a.shape[0], dtype=torch.float32, device=dev) for a in (sw.x, sw.y, sw.z)]
+    mine = sharding.tiles_of_rank(sw.tiles, rank, world)
+    geoms = [W.tile_geom(gk, *t) for t in mine]
+    bufs = [torch.empty((g.ny, g.nx), dtype=torch.float32, device=dev) for g in geoms]
+    failed = torch.zeros(1, dtype=torch.int64, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        sharding.broadcast_soundings(*xs, dist, 0)
+        idx = B.krige_build_index(*xs)
+        for g, bf in zip(geoms, bufs):
+            B.krige_predict(idx, g, sw.model, sw.range_, sw.sill, sw.nugget, sw.k, out=bf, failed=failed)
+        idx.free_async()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = B.launch_count()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = sharding.reduce_step_times([e0.elapsed_time(e1) / args.steps], dist, dev)[0]
+    assert int(failed.item()) == 0
+    if rank == 0:
+        print(json.dumps({"metric": "output nodes/s (ordinary kriging, one config-5 survey sharded by output tile)", "value": gk.n / (ms * 1e-3),
+                          "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+                          "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": WORKLOADS["config5"]["label"], "tiles_per_rank": len(mine),
+                                     "parallelism": f"replicated index (one broadcast of {12 * sw.x.shape[0] / 1e6:.0f} MB), output tiles round-robin x{world}"},
+                          "gpu_launches": int(B.launch_count() - n0)}))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import torch
     import paper_2505_22675_b200 as B
@@ -670,6 +731,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--no-extras", dest="extras", action="store_false",
                     help="skip the per-config table, the FP32 probe and e2e (short runs under ncu)")
+    ap.add_argument("--shard", default="batch", choices=["batch", "survey"],
+                    help="N > 1: every rank its own batch (weak, default) or ONE config-5 survey split by output tile (strong)")
     ap.add_argument("--reps", type=int, default=20, help="separately timed repetitions per method in the per-config table")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle work in cpu_baseline")
     args = ap.parse_args()
@@ -678,7 +741,10 @@ def main():
     else:
         if args.warmup < 3:
             args.warmup = 3                              # timing rule: W >= 3
-        run_ours(args)
+        if args.shard == "survey":
+            run_survey_sharded(args)
+        else:
+            run_ours(args)
 
 
 if __name__ == "__main__":

@@ -19,6 +19,22 @@ def tile_owner(tile_index: int, world: int) -> int:
     return int(tile_index) % max(int(world), 1)
 
 
+def tiles_of_rank(tiles, rank: int, world: int):
+    """The tiles of ONE survey that rank `rank` predicts (replicated index, output
+    tiles dealt round-robin in arrival order).  Every tile has exactly one owner."""
+    return [t for i, t in enumerate(tiles) if tile_owner(i, world) == int(rank)]
+
+
+def broadcast_soundings(x, y, z, dist=None, src: int = 0):
+    """Replicates the sounding set of rank `src` on every rank (one broadcast of <= 64 MB over NCCL / NVLink on
+    GPUs, gloo on CPU): the only data-plane communication of the one-survey sharding.  x, y, z: float32 tensors
+    of equal length on every rank (contents are only read on `src`).  Returns the three tensors."""
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        for t in (x, y, z):
+            dist.broadcast(t, src=src)
+    return x, y, z
+
+
 def reduce_step_times(times_ms, dist=None, device=None):
     """MAX over ranks of each entry of `times_ms` (list of floats).  `dist` is torch.distributed (or
     None for a single process)."""

@@ -76,6 +76,9 @@ def test_sharding_helpers():
     from paper_2505_22675_b200 import sharding as S
     assert S.rank_seed(1004, 0) == 1004 and S.rank_seed(1004, 3) == 1304
     assert [S.tile_owner(t, 4) for t in range(6)] == [0, 1, 2, 3, 0, 1]
+    tiles = list(range(64))
+    parts = [S.tiles_of_rank(tiles, r, 8) for r in range(8)]
+    assert sorted(sum(parts, [])) == tiles and all(len(p) == 8 for p in parts)
     assert S.whole_job_throughput(1000.0, 4, 2.0) == 2.0e6
     assert S.reduce_step_times([1.0, 2.0]) == [1.0, 2.0]
 
@@ -93,6 +96,16 @@ import torch
 chk = torch.tensor([float(w.x.sum())], dtype=torch.float64)
 gathered = [torch.zeros_like(chk) for _ in range(2)]
 dist.all_gather(gathered, chk)
+# one-survey sharding (NEXT-4): rank 0's soundings are replicated, the tiles are dealt round-robin
+w0 = W.sounding_config(5, width=60.0, n_target=900, n_out=32, seed=W.SEEDS[5])
+xs = [torch.from_numpy(a.copy()) if rank == 0 else torch.zeros(a.shape[0]) for a in (w0.x, w0.y, w0.z)]
+S.broadcast_soundings(*xs, dist, 0)
+assert all(torch.equal(t, torch.from_numpy(a)) for t, a in zip(xs, (w0.x, w0.y, w0.z)))
+tiles = W.boustrophedon_tiles(32, 8)
+mine = S.tiles_of_rank(tiles, rank, 2)
+cnt = torch.tensor([float(len(mine)), float(sum(t[2] * t[3] for t in mine))], dtype=torch.float64)
+dist.all_reduce(cnt)
+assert cnt.tolist() == [16.0, 1024.0], cnt
 dist.barrier()
 if rank == 0:
     assert ms == [15.0, 3.0], ms
