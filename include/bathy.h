@@ -282,6 +282,13 @@ BATHY_API int bathy_set_spline_path(int path);
 BATHY_API int bathy_probe_fp32(int32_t packed, int64_t iters, int32_t ctas_per_sm, float* d_sink, double* flop_out,
                      void* cuda_stream);
 
+/* TMA probe: loads the 88 x 54 fp32 box whose first element is column x0, row y0 of the
+ * [ny][nx] tensor d_in (nx and x0 multiples of 4, d_in 16-byte aligned; y0 is free) with ONE cp.async.bulk.tensor.2d into shared
+ * memory and copies it to d_out [54 * 88]; elements outside the tensor arrive as zeros.  The committed reproduction
+ * of whether TMA tensor loads work on the box.  Enqueue only; BATHY_ERR_CUDA if the tensor map cannot be encoded. */
+BATHY_API int bathy_probe_tma(const float* d_in, int32_t nx, int32_t ny, int32_t x0, int32_t y0, float* d_out,
+                    void* cuda_stream);
+
 /* Static, never NULL. */
 BATHY_API const char* bathy_strerror(int status);
 

@@ -26,7 +26,7 @@ SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_byt
            "interp_spline_host", "krige_host", "interp_bilinear_host_async", "interp_spline_host_async",
            "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path",
            "krige_predict_ex", "krige_index_create", "krige_index_append", "interp_catmull_rom_host",
-           "interp_catmull_rom_host_async", "bathy_probe_fp32", "interp_krige_window"]
+           "interp_catmull_rom_host_async", "bathy_probe_fp32", "interp_krige_window", "bathy_probe_tma"]
 
 
 class GridGeom(C.Structure):
@@ -93,6 +93,7 @@ def lib():
         L.bathy_strerror.restype = C.c_char_p
         L.bathy_launch_count.restype = C.c_int64
         L.bathy_set_spline_path.argtypes = [C.c_int]
+        L.bathy_probe_tma.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
         L.bathy_probe_fp32.argtypes = [C.c_int32, C.c_int64, C.c_int32, vp, C.POINTER(C.c_double), vp]
         _lib = L
     return _lib
@@ -132,6 +133,15 @@ def probe_fp32(packed: bool, iters: int, ctas_per_sm: int = 2, stream=None) -> f
     _check(lib().bathy_probe_fp32(int(bool(packed)), int(iters), int(ctas_per_sm), sink.data_ptr(), C.byref(flop),
                                   _stream(stream)), "bathy_probe_fp32")
     return float(flop.value)
+
+
+def probe_tma(z: torch.Tensor, x0: int, y0: int, stream=None) -> torch.Tensor:
+    """One cp.async.bulk.tensor.2d load of the 88 x 54 box at (x0, y0) of z [ny, nx] (include/bathy.h)."""
+    _dev_f32(z, "z")
+    out = torch.empty((54, 88), dtype=torch.float32, device=z.device)
+    _check(lib().bathy_probe_tma(z.data_ptr(), int(z.shape[1]), int(z.shape[0]), int(x0), int(y0), out.data_ptr(),
+                                 _stream(stream)), "bathy_probe_tma")
+    return out
 
 
 def set_spline_path(path: int) -> None:

@@ -319,3 +319,21 @@ def test_second_device_after_the_first_in_one_process():
     torch.cuda.set_device(0)
     for a, c in zip(*outs):
         assert torch.equal(a, c)
+
+
+def test_tma_tensor_load_probe():
+    """cp.async.bulk.tensor.2d (TMA) works on the box: one 88 x 54 box load, interior and clipped by the tensor edge
+    (out-of-tensor elements arrive as zeros).  The committed reproduction behind DESIGN.md's TMA paragraph: the
+    load works whenever the box's first COLUMN is a multiple of 4 floats (16 bytes), rows are free; a first column
+    that is not 16-byte aligned raises "illegal instruction" (profiles/r2_tma_probe.md) -- which is what round 1 hit."""
+    b = _bathy()
+    rng = np.random.default_rng(12)
+    z = rng.normal(size=(300, 512)).astype(np.float32)
+    zt = torch.from_numpy(z).cuda()
+    for x0, y0 in ((0, 0), (16, 33), (124, 200), (-12, -7), (468, 281), (-88, 3)):
+        got = b.probe_tma(zt, x0, y0).cpu().numpy()
+        want = np.zeros((54, 88), np.float32)
+        ys, xs = np.arange(y0, y0 + 54), np.arange(x0, x0 + 88)
+        oky, okx = (ys >= 0) & (ys < 300), (xs >= 0) & (xs < 512)
+        want[np.ix_(oky, okx)] = z[np.ix_(ys[oky], xs[okx])]
+        assert np.array_equal(got, want), (x0, y0)
