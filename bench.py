@@ -65,6 +65,8 @@ WORKLOADS = {
                     label="config2(bilinear+spline 1024^2->4093^2) + config4(kriging)"),
     "config5": dict(grid=(3, 4096, 2, 8000), krige=(5, 4000.0, 4_000_000, 4096), tiles=True,
                     label="config3(bilinear+spline) + config5(kriging 4.0M soundings->4096^2 as 64 tiles of 512^2, k=64 spherical)"),
+    "small5": dict(grid=(2, 257, 4, 40), krige=(5, 300.0, 22500, 128), tiles=True,
+                   label="reduced configs (257^2->1025^2; 22.5k soundings->128^2 as 64 tiles, k=64 spherical)"),
     "small": dict(grid=(2, 257, 4, 40), krige=(4, 250.0, 15625, 200), tiles=False,
                   label="reduced configs (257^2->1025^2; 15.6k soundings->200^2, k=32)"),
 }

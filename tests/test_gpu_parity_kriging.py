@@ -266,3 +266,29 @@ def test_async_host_forms_on_three_streams():
         ok.fill_(-1.0); ob.fill_(-1.0); os_.fill_(-1.0)
     with pytest.raises(TypeError):
         b.interp_bilinear_host_async(torch.from_numpy(gw.z), gw.geom_in, gw.geom_out, out=ob)      # not pinned
+
+
+@pytest.mark.parametrize("k,model", [(8, 1), (32, 0), (64, 1)])
+def test_repeated_launches_are_bit_identical(k, model):
+    """Stands in for racecheck (closed on the pool, profiles/r2_sanitizer_refusal.md): a data race in the
+    __syncwarp-ordered shared-memory buffers of the solve would make the result timing dependent; 12 launches, with
+    another stream keeping the SMs busy, give bit-identical depths and variances."""
+    b = _bathy()
+    w = W.sounding_config(4, width=200.0, n_target=10000, n_out=160)
+    xt, yt, zt = (torch.from_numpy(a).cuda() for a in (w.x, w.y, w.z))
+    idx = b.krige_build_index(xt, yt, zt)
+    side = torch.cuda.Stream()
+    noise = torch.randn(2048, 2048, device="cuda")
+    first = None
+    for it in range(12):
+        with torch.cuda.stream(side):
+            for _ in range(it % 4):
+                noise = torch.tanh(noise @ noise * 1e-3)
+        z, var = b.krige_predict(idx, w.geom_out, model, 60.0, w.sill, w.nugget, k, want_var=True)
+        if first is None:
+            first = (z.clone(), var.clone())
+        else:
+            assert torch.equal(z, first[0]) and torch.equal(var, first[1])
+    torch.cuda.synchronize()
+    idx.free()
+    assert torch.isfinite(first[0]).all()
