@@ -268,7 +268,8 @@ BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* 
  * 0 = automatic (default): the fused single-pass tile kernel where it applies (up-sampling, input at
  *     least one solve window wide), else the global-solve path;
  * 1 = fused tile kernel only (BATHY_ERR_GEOMETRY where it does not apply);
- * 2 = global-solve path only (three batched full-length Thomas solves + gather evaluate).
+ * 2 = global-solve path only (three batched full-length Thomas solves + gather evaluate);
+ * 3 = fused tile kernel with the window staged by cp.async instead of the TMA box load (profiling A/B).
  * Both compute the same natural bicubic spline; DESIGN.md "Spline window bound" gives the bound on
  * their difference (8.2e-7 x depth range per direction). */
 BATHY_API int bathy_set_spline_path(int path);

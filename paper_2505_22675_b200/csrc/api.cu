@@ -302,7 +302,7 @@ BATHY_API const char* bathy_strerror(int status)
 
 BATHY_API int bathy_set_spline_path(int path)
 {
-    if (path < 0 || path > 2) return BATHY_ERR_GEOMETRY;
+    if (path < 0 || path > 3) return BATHY_ERR_GEOMETRY;
     g_spline_path.store(path);
     return BATHY_OK;
 }

@@ -94,7 +94,7 @@ spline_eval_kernel(const float* __restrict__ z, const float* __restrict__ Mx, co
 }  // namespace
 
 size_t spline_tiled_table_bytes(const grid_geom_t&, const grid_geom_t&);                                      // spline_tile.cu
-int launch_spline_tiled(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t);   // spline_tile.cu
+int launch_spline_tiled(const float*, const grid_geom_t&, float*, const grid_geom_t&, void*, cudaStream_t, bool allow_tma);   // spline_tile.cu
 
 // Workspace: the axis tables of the fused path, then the three second-derivative planes of the
 // global-solve path.
@@ -108,10 +108,10 @@ size_t spline_workspace_bytes(const grid_geom_t& in, const grid_geom_t& out)
 int launch_spline(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
                   void* d_ws, cudaStream_t stream, int path)
 {
-    if (path != 2) {                                   // 0 = automatic, 1 = fused tiles only, 2 = global solves only
-        const int rc = launch_spline_tiled(d_in, in, d_out, out, d_ws, stream);
+    if (path != 2) {                                   // 0 = automatic, 1 / 3 = fused tiles only (3: no TMA), 2 = global solves only
+        const int rc = launch_spline_tiled(d_in, in, d_out, out, d_ws, stream, path != 3);
         if (rc != 1) return rc;
-        if (path == 1) return BATHY_ERR_GEOMETRY;
+        if (path == 1 || path == 3) return BATHY_ERR_GEOMETRY;
     }
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
     const size_t n = (size_t)in.nx * (size_t)in.ny;

@@ -22,8 +22,10 @@
 // the grid spacing drops out of the arithmetic.
 // HBM traffic: the input once (window halos are L2 hits), the output once = the compulsory bytes.
 #include <type_traits>
+#include <string.h>
 
 #include "common.cuh"
+#include "tma.cuh"
 
 namespace bathy {
 
@@ -54,7 +56,8 @@ struct TileShape {
     static constexpr int front_floats = (4 * NYI * PQ > WY * PA) ? 4 * NYI * PQ : WY * PA;   // max(knot records, raw window)
     static constexpr int PSK = (16 - (NYI * PZ) % 32 + 32) % 32;   // skew of the second plane: the two planes of a
                                                        // knot row sit 16 banks apart (x sweeps, below)
-    static constexpr size_t smem_bytes = sizeof(float) * ((size_t)front_floats + 2 * (size_t)NYI * PZ + PSK);
+    static constexpr size_t data_bytes = (sizeof(float) * ((size_t)front_floats + 2 * (size_t)NYI * PZ + PSK) + 15) / 16 * 16;
+    static constexpr size_t smem_bytes = data_bytes + 16;             // + the mbarrier of the TMA window load
     static_assert(WX <= kTileThreads && 2 * NYI <= kTileThreads && NYI <= 32, "tile shape");
 };
 
@@ -181,12 +184,13 @@ __global__ void __launch_bounds__(kTileThreads, 4)
 spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay,
                    const float4* __restrict__ colw, const float4* __restrict__ rowtab,
                    const int* __restrict__ tbx, const int* __restrict__ tby, const int* __restrict__ rfirst,
-                   const int* __restrict__ coli, int nbx, int n_tiles, int pf_dist)
+                   const int* __restrict__ coli, int nbx, int n_tiles, int pf_dist,
+                   const __grid_constant__ CUtensorMap tmap, int use_tma)
 {
     constexpr int TXI = S::TXI, TYI = S::TYI, H = S::H, WX = S::WX, WY = S::WY;
     constexpr int NXI = S::NXI, NYI = S::NYI, PZ = S::PZ, PA = S::PA, PQ = S::PQ;
     constexpr int NW = kTileThreads / 32;
-    extern __shared__ __align__(16) unsigned char s_raw[];
+    extern __shared__ __align__(128) unsigned char s_raw[];
     // The raw window is dead once the y sweep has run, the knot records are born after it: they share
     // the front of the buffer (55 KB per CTA: four CTAs per SM).
     float4* s_q = reinterpret_cast<float4*>(s_raw);                       // [NYI][PQ] knot records (z, Mx', My', Mxy')
@@ -238,8 +242,20 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const int w0y = min(max(j0 - H, 0), ay.n_in - WY);
         const int kx0 = i0 - w0x, ky0 = j0 - w0y;                         // tile knot 0 in window coordinates
         const int nkx = min(NXI, ax.n_in - i0), nky = min(NYI, ay.n_in - j0);   // knots present (last tile may be short)
-        issue_load(tile, 0);
-        asm volatile("cp.async.commit_group;" ::: "memory");
+        // The window goes global -> shared in ONE TMA box load (cp.async.bulk.tensor.2d: no LSU wavefronts, no
+        // per-thread address arithmetic) when the input rows are 16-byte aligned; the box starts at the aligned
+        // column at or before the window start (profiles/r2_tma_probe.md), columns past the row end arrive as
+        // zeros.  Otherwise by cp.async / plain loads.
+        const unsigned bar = (unsigned)__cvta_generic_to_shared(s_raw + S::data_bytes);
+        if (use_tma) {
+            if (tid == 0) {
+                mbar_init(bar, 1);
+                tma_load_2d((unsigned)__cvta_generic_to_shared(s_zbuf), &tmap, w0x & ~3, w0y, bar, (unsigned)(WY * PA * sizeof(float)));
+            }
+        } else {
+            issue_load(tile, 0);
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
         {
             // L2 prefetch of the window of the tile that starts one wave of CTAs later: its cp.async
             // then finds the rows in L2 instead of waiting for HBM at the head of the CTA
@@ -266,8 +282,13 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
         const int kja = warp * TI, kjb = min(min(kja + TI, TYI), nky - 1);
         const int rb = min(max(__ldg(rfirst + min(j0 + kja, ay.n_in)), Ibeg), Iend);
         const int re = (kjb > kja) ? min(max(__ldg(rfirst + min(j0 + kjb, ay.n_in)), Ibeg), Iend) : rb;
-        asm volatile("cp.async.wait_group 0;" ::: "memory");             // the window has landed
-        __syncthreads();
+        if (use_tma) {
+            __syncthreads();                                             // the barrier is initialised
+            mbar_wait(bar, 0);                                           // the window has landed
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");         // the window has landed
+            __syncthreads();
+        }
         float zref = s_z[offx];                                           // the window's first sample
         if (!isfinite(zref)) zref = 0.0f;
         // the table entries the evaluate stage starts with: into L1 now, two stages ahead of their use
@@ -446,7 +467,7 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
 }
 
 template <class S>
-int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMap& ay, void* d_ws, cudaStream_t stream)
+int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMap& ay, void* d_ws, cudaStream_t stream, bool allow_tma)
 {
     static DeviceOnce once;
     const int rc_attr = once_per_device(once, []() -> int {
@@ -468,6 +489,11 @@ int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMa
     const long long n_tiles = (long long)grid.x * grid.y;
     if (n_tiles > 0x7fffffffLL) return 1;
     const unsigned ctas = (unsigned)n_tiles;
+    CUtensorMap tmap;
+    memset(&tmap, 0, sizeof(tmap));
+    int use_tma = 0;
+    if (allow_tma && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (ax.n_in & 3) == 0)
+        use_tma = tensor_map_2d(&tmap, d_in, ax.n_in, ay.n_in, S::PA, S::WY) == BATHY_OK ? 1 : 0;
     {
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(ctas);
@@ -481,7 +507,7 @@ int launch_tile(const float* d_in, float* d_out, const AxisMap& ax, const AxisMa
         cfg.numAttrs = 1;
         BATHY_CUDA_TRY(cudaLaunchKernelEx(&cfg, spline_tile_kernel<S>, d_in, d_out, ax, ay, (const float4*)colw, (const float4*)rowtab,
                                           (const int*)tbx, (const int*)tby, (const int*)rfirst, (const int*)coli,
-                                          (int)grid.x, (int)n_tiles, 4 * kSMs /* CTAs resident at once */));
+                                          (int)grid.x, (int)n_tiles, 4 * kSMs /* CTAs resident at once */, tmap, use_tma));
     }
     count_launch(2);
     return launch_status();
@@ -499,7 +525,7 @@ size_t spline_tiled_table_bytes(const grid_geom_t& in, const grid_geom_t& out)
 }
 
 int launch_spline_tiled(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
-                        void* d_ws, cudaStream_t stream)
+                        void* d_ws, cudaStream_t stream, bool allow_tma)
 {
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
     // up-sampling (or 1:1) only: a tile must produce at least about as many nodes as it reads knots
@@ -508,9 +534,9 @@ int launch_spline_tiled(const float* d_in, const grid_geom_t& in, float* d_out, 
     using Small = TileShape<16, 16, 11>;
     if (in.nx >= Big::WX && in.ny >= Big::WY) {
         if ((in.ny - 1 + Big::TYI - 1) / Big::TYI > 65535) return 1;
-        return launch_tile<Big>(d_in, d_out, ax, ay, d_ws, stream);
+        return launch_tile<Big>(d_in, d_out, ax, ay, d_ws, stream, allow_tma);
     }
-    if (in.nx >= Small::WX && in.ny >= Small::WY) return launch_tile<Small>(d_in, d_out, ax, ay, d_ws, stream);
+    if (in.nx >= Small::WX && in.ny >= Small::WY) return launch_tile<Small>(d_in, d_out, ax, ay, d_ws, stream, allow_tma);
     return 1;
 }
 

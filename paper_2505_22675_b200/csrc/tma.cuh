@@ -1,0 +1,56 @@
+// tma.cuh -- the few lines of TMA (cp.async.bulk.tensor) plumbing the grid kernels share: a 2-D fp32 tensor map of
+// the input grid (host), and the mbarrier / load / wait sequence of ONE tile load (device).  Rules measured on the
+// pool's B200s (profiles/r2_tma_probe.md): box rows a multiple of 16 bytes, the box's first column a multiple of
+// 4 floats, 128-byte aligned shared-memory destination; elements outside the tensor arrive as zeros.
+#pragma once
+#include <cuda.h>
+#include "common.cuh"
+
+namespace bathy {
+
+// Tensor map of the row-major [ny][nx] fp32 grid `base` with a box of box_w x box_h elements.  Needs nx % 4 == 0
+// and a 16-byte aligned base (the caller checks); BATHY_ERR_CUDA if the driver refuses.
+inline int tensor_map_2d(CUtensorMap* map, const float* base, int nx, int ny, int box_w, int box_h)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static std::atomic<void*> cached{nullptr};
+    void* fn = cached.load(std::memory_order_acquire);
+    if (!fn) {
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+            qres != cudaDriverEntryPointSuccess) { cudaGetLastError(); return BATHY_ERR_CUDA; }
+        cached.store(fn, std::memory_order_release);
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)nx, (cuuint64_t)ny};
+    const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(float)};
+    const cuuint32_t box[2] = {(cuuint32_t)box_w, (cuuint32_t)box_h};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = reinterpret_cast<encode_fn>(fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides,
+                                                       box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                       CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? BATHY_OK : BATHY_ERR_CUDA;
+}
+
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+// One elected thread: announce `bytes` and start the box load whose first element is (x, y) (x % 4 == 0).
+__device__ __forceinline__ void tma_load_2d(unsigned dst, const CUtensorMap* map, int x, int y, unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 :: "r"(dst), "l"(map), "r"(x), "r"(y), "r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra WAIT_%=;\n\t}"
+                 :: "r"(bar), "r"(parity) : "memory");
+}
+
+}  // namespace bathy
