@@ -219,3 +219,24 @@ def test_spline_fused_path_refuses_what_it_cannot_serve(spline_path):
         b.interp_spline(z, W.Geom(20, 20, 0, 0, 1, 1), W.Geom(39, 39, 0, 0, .5, .5))
     spline_path(0)
     b.interp_spline(z, W.Geom(20, 20, 0, 0, 1, 1), W.Geom(39, 39, 0, 0, .5, .5))   # automatic: global path
+
+
+@pytest.mark.parametrize("ny,nx", [(600, 777), (257, 1025), (513, 33), (40, 300)])
+def test_spline_global_path_segments_worst_case(spline_path, ny, nx):
+    """The global-solve path cuts every system into 256-knot segments solved on windows with a 32-knot halo
+    (0.268^32 = 5e-19: below fp32 rounding): sizes with several ragged segments per direction, on full-amplitude
+    white noise (the largest second derivatives a depth range allows), down- and up-sampling, TMA and cp.async paths."""
+    rng = np.random.default_rng(1000 + nx)
+    z = rng.uniform(-6000, -5000, (ny, nx)).astype(np.float32)
+    gi = W.Geom(nx, ny, 0.0, 0.0, 1.0, 1.0)
+    for go in (W.Geom(2 * nx - 1, 2 * ny - 1, 0.0, 0.0, 0.5, 0.5), W.Geom(nx // 2, ny // 3, 0.3, 0.7, 1.9, 2.7)):
+        ref = _ref("spline", z, gi, go)
+        spline_path(2)
+        got = _run("spline", z, gi, go)
+        assert max_abs_err(got, ref) <= TOL * depth_range(ref), (ny, nx, go)
+    if nx >= 87 and ny >= 54:
+        go = W.Geom(2 * nx - 1, 2 * ny - 1, 0.0, 0.0, 0.5, 0.5)
+        ref = _ref("spline", z, gi, go)
+        for path in (1, 3):
+            spline_path(path)
+            assert max_abs_err(_run("spline", z, gi, go), ref) <= TOL * depth_range(ref), path
