@@ -52,25 +52,9 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
     // The footprint goes global -> shared by cp.async, all of it in flight at once (16-byte vectors
     // from the aligned column at or before i_lo when the rows are 16-byte aligned); the double-precision
     // column maps below are computed while it streams in.
-    const int a_lo = i_lo & ~3, offx = i_lo - a_lo;
-    const int pitch = (fw + 6) & ~3;                  // >= offx + fw, a multiple of 4
-    if ((reinterpret_cast<uintptr_t>(in) & 15) == 0 && (ax.n_in & 3) == 0) {
-        const int vpr = pitch >> 2;
-        for (int v = tid; v < fh * vpr; v += kThreads) {
-            const int r = v / vpr, c4 = (v - r * vpr) << 2;
-            const int col = a_lo + c4;
-            const int bytes = max(0, min(16, (ax.n_in - col) * 4));      // past the row end: zero fill
-            const float* src = in + (size_t)(j_lo + r) * ax.n_in + min(col, ax.n_in - 4);
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + c4);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(bytes) : "memory");
-        }
-    } else {
-        for (int v = tid; v < fh * fw; v += kThreads) {
-            const int r = v / fw, c = v - r * fw;
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + offx + c);
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(dst), "l"(in + (size_t)(j_lo + r) * ax.n_in + i_lo + c) : "memory");
-        }
-    }
+    const int offx = i_lo & 3;
+    const int pitch = stage_pitch(fw);
+    stage_footprint(in, ax.n_in, i_lo, j_lo, fw, fh, s_tile, tid, kThreads);
     asm volatile("cp.async.commit_group;" ::: "memory");
     float zref = __ldg(in + (size_t)j_lo * ax.n_in + i_lo);
     if (!isfinite(zref)) zref = 0.0f;

@@ -62,25 +62,9 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     const int fj0 = max(s_bounds[2] - 1, 0), fj1 = min(s_bounds[3] + 1, ay.n_in - 1);
     const int fw = fi1 - fi0 + 1, fh = fj1 - fj0 + 1;
 
-    const int a_lo = fi0 & ~3, offx = fi0 - a_lo;
-    const int pitch = (fw + 6) & ~3;                  // >= offx + fw, a multiple of 4
-    if ((reinterpret_cast<uintptr_t>(in) & 15) == 0 && (ax.n_in & 3) == 0) {
-        const int vpr = pitch >> 2;
-        for (int v = tid; v < fh * vpr; v += kThreads) {
-            const int r = v / vpr, c4 = (v - r * vpr) << 2;
-            const int col = a_lo + c4;
-            const int bytes = max(0, min(16, (ax.n_in - col) * 4));      // past the row end: zero fill
-            const float* src = in + (size_t)(fj0 + r) * ax.n_in + min(col, ax.n_in - 4);
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + c4);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(bytes) : "memory");
-        }
-    } else {
-        for (int v = tid; v < fh * fw; v += kThreads) {
-            const int r = v / fw, c = v - r * fw;
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + offx + c);
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(dst), "l"(in + (size_t)(fj0 + r) * ax.n_in + fi0 + c) : "memory");
-        }
-    }
+    const int offx = fi0 & 3;
+    const int pitch = stage_pitch(fw);
+    stage_footprint(in, ax.n_in, fi0, fj0, fw, fh, s_tile, tid, kThreads);
     asm volatile("cp.async.commit_group;" ::: "memory");
     float zref = __ldg(in + (size_t)fj0 * ax.n_in + fi0);
     if (!isfinite(zref)) zref = 0.0f;

@@ -107,6 +107,37 @@ inline long long footprint_bound(const AxisMap& m, int n_nodes)
 }
 
 
+// Stages rows [j0, j0 + fh) x columns [i0, i0 + fw) of the row-major input (leading dimension n_in) in shared
+// memory by cp.async, ALL of it in flight at once; the caller commits / waits.  Row r of the footprint starts at
+// s_tile + r * pitch + offx, where pitch = stage_pitch(fw) and offx = i0 & 3: with 16-byte aligned input rows the
+// copy runs in whole 16-byte vectors from the aligned column at or before i0 (columns past the row end are zero
+// filled), else element by element.  Shared by the bilinear and Catmull-Rom tile kernels.
+__host__ __device__ __forceinline__ int stage_pitch(int fw) { return (fw + 6) & ~3; }   // >= (i0 & 3) + fw, a multiple of 4
+
+__device__ __forceinline__ void stage_footprint(const float* __restrict__ in, int n_in, int i0, int j0, int fw, int fh,
+                                                float* s_tile, int tid, int nthreads)
+{
+    const int a_lo = i0 & ~3, offx = i0 - a_lo;
+    const int pitch = stage_pitch(fw);
+    if ((reinterpret_cast<uintptr_t>(in) & 15) == 0 && (n_in & 3) == 0) {
+        const int vpr = pitch >> 2;
+        for (int v = tid; v < fh * vpr; v += nthreads) {
+            const int r = v / vpr, c4 = (v - r * vpr) << 2;
+            const int col = a_lo + c4;
+            const int bytes = max(0, min(16, (n_in - col) * 4));         // past the row end: zero fill
+            const float* src = in + (size_t)(j0 + r) * n_in + min(col, n_in - 4);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + c4);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(bytes) : "memory");
+        }
+    } else {
+        for (int v = tid; v < fh * fw; v += nthreads) {
+            const int r = v / fw, c = v - r * fw;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_tile + r * pitch + offx + c);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" :: "r"(dst), "l"(in + (size_t)(j0 + r) * n_in + i0 + c) : "memory");
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Packed fp32x2 arithmetic of sm_100 (SASS FFMA2 / FMUL2 / FADD2): one issue slot, two fp32
 // operations.  A pair lives in a 64-bit register; a scalar operand packed as (a, a) is folded by
