@@ -21,6 +21,7 @@ int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, i
 int launch_krige_window(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
                         cudaStream_t);
 
+extern bool g_bilinear_tma;
 static std::atomic<int64_t> g_launches{0};
 static std::atomic<int> g_spline_path{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
@@ -304,6 +305,7 @@ BATHY_API int bathy_set_spline_path(int path)
 {
     if (path < 0 || path > 3) return BATHY_ERR_GEOMETRY;
     g_spline_path.store(path);
+    g_bilinear_tma = (path != 3);
     return BATHY_OK;
 }
 

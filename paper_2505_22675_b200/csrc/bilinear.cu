@@ -12,6 +12,8 @@
 // recomputed only when the output row enters a new input interval, so a node costs half a packed FMA,
 // half a packed add (z_ref, added last) and one store plus its share of the per-row and per-interval work.
 #include "common.cuh"
+#include "tma.cuh"
+#include <string.h>
 
 namespace bathy {
 
@@ -19,12 +21,20 @@ namespace {
 
 constexpr int kThreads = 256;
 
-template <int CPT, int TH>
+constexpr int kBoxW = 64;                            // columns of one TMA box of the footprint
+
+// TMA = true (input rows 16-byte aligned): the footprint arrives as ceil(width / 64) TMA boxes of 64 columns x box_h
+// rows (cp.async.bulk.tensor.2d: one elected thread, no per-thread address arithmetic, no LSU wavefronts), box b at
+// s_tile + b * box_h * 64; sample (row r, column c) of the footprint sits at (c / 64) * box_h * 64 + r * 64 + c % 64.
+// TMA = false: cp.async into [fh][pitch] (common.cuh stage_footprint).
+template <int CPT, int TH, bool TMA>
 __global__ void __launch_bounds__(kThreads)
-bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay)
+bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay,
+                      const __grid_constant__ CUtensorMap tmap, int box_h)
 {
     constexpr int TW = CPT * kThreads;
-    extern __shared__ __align__(16) float s_tile[];   // [fh][pitch] raw input samples of the tile's footprint
+    extern __shared__ __align__(128) float s_tile[];  // raw input samples of the tile's footprint
+    __shared__ __align__(8) unsigned long long s_bar; // mbarrier of the TMA loads
     __shared__ int2  s_row[TH];                       // (input row j or -1, float bits of s) per output row
     __shared__ int   s_bounds[4];                     // i_lo, i_hi, j_lo, j_hi (sample indices)
 
@@ -53,9 +63,21 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
     // from the aligned column at or before i_lo when the rows are 16-byte aligned); the double-precision
     // column maps below are computed while it streams in.
     const int offx = i_lo & 3;
-    const int pitch = stage_pitch(fw);
-    stage_footprint(in, ax.n_in, i_lo, j_lo, fw, fh, s_tile, tid, kThreads);
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    const int pitch = TMA ? kBoxW : stage_pitch(fw);  // floats between consecutive footprint rows
+    const unsigned bar = (unsigned)__cvta_generic_to_shared(&s_bar);
+    if (TMA) {
+        if (tid == 0) {
+            const int nb = (offx + fw + kBoxW - 1) / kBoxW;
+            const unsigned box_bytes = (unsigned)(box_h * kBoxW * sizeof(float));
+            mbar_init(bar, 1);
+            mbar_expect(bar, box_bytes * nb);
+            for (int b = 0; b < nb; ++b)
+                tma_issue_2d((unsigned)__cvta_generic_to_shared(s_tile) + b * box_bytes, &tmap, (i_lo & ~3) + b * kBoxW, j_lo, bar);
+        }
+    } else {
+        stage_footprint(in, ax.n_in, i_lo, j_lo, fw, fh, s_tile, tid, kThreads);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
     float zref = __ldg(in + (size_t)j_lo * ax.n_in + i_lo);
     if (!isfinite(zref)) zref = 0.0f;
 
@@ -69,19 +91,32 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
         ct[e] = 0.0f;
         ci[e] = (J <= Jlast) ? axis_locate(ax, J, &ct[e]) : -1;
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    __syncthreads();
+    if (TMA) {
+        __syncthreads();                                  // the barrier is initialised
+        mbar_wait(bar, 0);                                // the footprint has landed
+    } else {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+    }
 
     const float qnan = __int_as_float(0x7fc00000);
     static_assert(CPT % 2 == 0, "columns are processed as fp32x2 pairs");
     bool cok[CPT];                                    // column is inside the tile (store predicate)
     float cz[CPT];                                    // z_ref, or NaN for a column outside the input extent
-    int   cofs[CPT];                                  // offset of the interval's left sample in a tile row
+    int   cofl[CPT], cofr[CPT];                       // offsets of the interval's left / right sample from the start of its footprint row
 #pragma unroll
     for (int e = 0; e < CPT; ++e) {
         cok[e] = (Jt + 32 * e) <= Jlast;
         cz[e] = (ci[e] < 0) ? qnan : zref;
-        cofs[e] = max(ci[e] - i_lo, 0) + offx;
+        const int c = max(ci[e] - i_lo, 0) + offx;
+        if (TMA) {
+            const int bs = box_h * kBoxW;
+            cofl[e] = (c / kBoxW) * bs + (c % kBoxW);
+            cofr[e] = ((c + 1) / kBoxW) * bs + ((c + 1) % kBoxW);
+        } else {
+            cofl[e] = c;
+            cofr[e] = c + 1;
+        }
     }
 
     // Two columns to a 64-bit register pair: a node is half a packed FMA (FFMA2) and a store.
@@ -100,8 +135,7 @@ bilinear_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, Axi
     auto hrow = [&](const float* row, u64* h2) {
 #pragma unroll
         for (int p = 0; p < CPT / 2; ++p) {
-            const int c0 = cofs[2 * p], c1 = cofs[2 * p + 1];
-            const u64 l = pack2(row[c0], row[c1]), r = pack2(row[c0 + 1], row[c1 + 1]);
+            const u64 l = pack2(row[cofl[2 * p]], row[cofl[2 * p + 1]]), r = pack2(row[cofr[2 * p]], row[cofr[2 * p + 1]]);
             h2[p] = ffma2(ct2[p], ffma2(l, neg1, r), fadd2(l, nzref2));
         }
     };
@@ -183,23 +217,38 @@ bilinear_gather_kernel(const float* __restrict__ in, float* __restrict__ out, Ax
 
 }  // namespace
 
+bool g_bilinear_tma = true;   // A/B switch (bathy_set_spline_path(3) turns the TMA staging of the grid kernels off)
+
 int launch_bilinear(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
                     cudaStream_t stream)
 {
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
     constexpr int CPT = 4, TH = 32, TW = CPT * kThreads;
     const long long fw = footprint_bound(ax, TW), fh = footprint_bound(ay, TH);
-    const long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
+    long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
+    // TMA staging when the input rows are 16-byte aligned and the box fits (box height <= 256): the footprint as
+    // boxes of 64 columns x fh rows
+    CUtensorMap tmap;
+    memset(&tmap, 0, sizeof(tmap));
+    const long long nbox = (fw + 3 + kBoxW - 1) / kBoxW;
+    const long long smem_tma = nbox * fh * kBoxW * (long long)sizeof(float);
+    bool use_tma = g_bilinear_tma && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (in.nx & 3) == 0 && fh <= 256 &&
+                   smem_tma <= 160 * 1024 && in.nx >= kBoxW;
+    if (use_tma) use_tma = tensor_map_2d(&tmap, d_in, in.nx, in.ny, kBoxW, (int)fh) == BATHY_OK;
+    if (use_tma) smem = smem_tma;
     if (smem <= 160 * 1024 && (out.ny + TH - 1) / TH <= 65535) {
         static DeviceOnce once;
         const int rc = once_per_device(once, []() -> int {
-            BATHY_CUDA_TRY(cudaFuncSetAttribute(bilinear_tiled_kernel<CPT, TH>,
+            BATHY_CUDA_TRY(cudaFuncSetAttribute(bilinear_tiled_kernel<CPT, TH, true>,
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+            BATHY_CUDA_TRY(cudaFuncSetAttribute(bilinear_tiled_kernel<CPT, TH, false>,
                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
             return (int)BATHY_OK;
         });
         if (rc) return rc;
         dim3 grid((out.nx + TW - 1) / TW, (out.ny + TH - 1) / TH);
-        bilinear_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay);
+        if (use_tma) bilinear_tiled_kernel<CPT, TH, true><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay, tmap, (int)fh);
+        else         bilinear_tiled_kernel<CPT, TH, false><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay, tmap, 0);
     } else {
         dim3 grid((out.nx + kThreads - 1) / kThreads, out.ny < 65535 ? out.ny : 65535);
         bilinear_gather_kernel<<<grid, kThreads, 0, stream>>>(d_in, d_out, ax, ay);
