@@ -14,6 +14,8 @@
 // algebra):  w0 = (-t + 2t^2 - t^3)/2, w1 = (2 - 5t^2 + 3t^3)/2, w2 = (t + 4t^2 - 3t^3)/2,
 // w3 = (-t^2 + t^3)/2.
 #include "common.cuh"
+#include "tma.cuh"
+#include <string.h>
 
 namespace bathy {
 
@@ -28,12 +30,16 @@ __device__ __forceinline__ float4 cr_weights(float t)
                        0.5f * (t + 4.0f * t2 - 3.0f * t3), 0.5f * (-t2 + t3));
 }
 
-template <int CPT, int TH>
+constexpr int kBoxW = 64;                            // columns of one TMA box of the footprint (layout: see bilinear.cu)
+
+template <int CPT, int TH, bool TMA>
 __global__ void __launch_bounds__(kThreads, 3)
-catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay)
+catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMap ax, AxisMap ay,
+                         const __grid_constant__ CUtensorMap tmap, int box_h)
 {
     constexpr int TW = CPT * kThreads;
-    extern __shared__ __align__(16) float s_tile[];   // [fh][pitch] raw input samples of the tile's footprint
+    extern __shared__ __align__(128) float s_tile[];  // raw input samples of the tile's footprint
+    __shared__ __align__(8) unsigned long long s_bar; // mbarrier of the TMA loads
     __shared__ float4 s_wy[TH];                       // y weights of the output row
     __shared__ int2   s_row[TH];                      // (input row j or -1, float bits of s) per output row
     __shared__ int    s_bounds[4];                    // i_lo, i_hi, j_lo, j_hi (interval bounds of the tile)
@@ -63,9 +69,24 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     const int fw = fi1 - fi0 + 1, fh = fj1 - fj0 + 1;
 
     const int offx = fi0 & 3;
-    const int pitch = stage_pitch(fw);
-    stage_footprint(in, ax.n_in, fi0, fj0, fw, fh, s_tile, tid, kThreads);
-    asm volatile("cp.async.commit_group;" ::: "memory");
+    const int pitch = TMA ? kBoxW : stage_pitch(fw);  // floats between consecutive footprint rows
+    const int bs = box_h * kBoxW;                     // floats between consecutive boxes
+    const unsigned bar = (unsigned)__cvta_generic_to_shared(&s_bar);
+    if (TMA) {
+        if (tid == 0) {
+            const int nb = (offx + fw + kBoxW - 1) / kBoxW;
+            const unsigned box_bytes = (unsigned)(bs * sizeof(float));
+            mbar_init(bar, 1);
+            mbar_expect(bar, box_bytes * nb);
+            for (int b = 0; b < nb; ++b)
+                tma_issue_2d((unsigned)__cvta_generic_to_shared(s_tile) + b * box_bytes, &tmap, (fi0 & ~3) + b * kBoxW, fj0, bar);
+        }
+    } else {
+        stage_footprint(in, ax.n_in, fi0, fj0, fw, fh, s_tile, tid, kThreads);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+    // byte offset of footprint column c (counted from the aligned start) inside a footprint row
+    auto boff = [&](int c) { return TMA ? 4u * (unsigned)((c / kBoxW) * bs + (c % kBoxW)) : 4u * (unsigned)c; };
     float zref = __ldg(in + (size_t)fj0 * ax.n_in + fi0);
     if (!isfinite(zref)) zref = 0.0f;
 
@@ -74,8 +95,8 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
     bool cok[CPT], c4ok[CPT];                         // column inside the tile / has its 4 x neighbours in the grid
     float ct[CPT], cnan[CPT];
     float cw0[CPT], cw2[CPT], cw3[CPT];               // x weights of P0, P2, P3 (P1's is 1 minus their sum)
-    unsigned o1[CPT], o0[CPT], o3[CPT];               // byte offsets of P1, P0, P3 in a footprint row (P2 at o1 + 4; P0 and
-                                                      // P3 clamped into the footprint): a shared-memory address is one add
+    unsigned o1[CPT], o0[CPT], o2[CPT], o3[CPT];      // byte offsets of P1, P0, P2, P3 in a footprint row (P0 and P3 clamped
+                                                      // into the footprint): a shared-memory address is one add
     const float qnan = __int_as_float(0x7fc00000);
 #pragma unroll
     for (int e = 0; e < CPT; ++e) {
@@ -89,15 +110,20 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
         const float4 w = cr_weights(ct[e]);
         cw0[e] = w.x; cw2[e] = w.z; cw3[e] = w.w;
         const int c1 = min(max(ic, fi0), fi1 - 1) - fi0 + offx;
-        o1[e] = 4u * (unsigned)c1;
-        o0[e] = (c1 - 1 >= offx) ? o1[e] - 4u : o1[e];
-        o3[e] = (c1 + 2 <= fi1 - fi0 + offx) ? o1[e] + 8u : o1[e] + 4u;
+        o1[e] = boff(c1);
+        o2[e] = boff(c1 + 1);
+        o0[e] = (c1 - 1 >= offx) ? boff(c1 - 1) : o1[e];
+        o3[e] = (c1 + 2 <= fi1 - fi0 + offx) ? boff(c1 + 2) : o2[e];
     }
     const unsigned tile_sa = (unsigned)__cvta_generic_to_shared(s_tile);
     auto lds = [](unsigned a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); return v; };
-    auto lds4 = [](unsigned a) { float v; asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(v) : "r"(a) : "memory"); return v; };
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    __syncthreads();
+    if (TMA) {
+        __syncthreads();                                  // the barrier is initialised
+        mbar_wait(bar, 0);                                // the footprint has landed
+    } else {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+    }
 
     // x cubic of input row jrow at this thread's columns, on (sample - z_ref), two columns to a pair.  With
     // w1 = 1 - w0 - w2 - w3 the cubic is P1 + w0 (P0 - P1) + w2 (P2 - P1) + w3 (P3 - P1): differences of
@@ -126,7 +152,7 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
             const u64 p1 = pack2(lds(qa), lds(qb));
             const u64 np1 = fmul2(p1, neg1);
             const u64 d0 = fadd2(pack2(lds(row + o0[2 * p]), lds(row + o0[2 * p + 1])), np1);
-            const u64 d2 = fadd2(pack2(lds4(qa), lds4(qb)), np1);
+            const u64 d2 = fadd2(pack2(lds(row + o2[2 * p]), lds(row + o2[2 * p + 1])), np1);
             const u64 d3 = fadd2(pack2(lds(row + o3[2 * p]), lds(row + o3[2 * p + 1])), np1);
             X2[p] = ffma2(w3x[p], d3, ffma2(w2x[p], d2, ffma2(w0x[p], d0, fadd2(p1, nzr[p]))));
         }
@@ -140,7 +166,7 @@ catmull_rom_tiled_kernel(const float* __restrict__ in, float* __restrict__ out, 
 #pragma unroll
         for (int e = 0; e < CPT; ++e) {
             const float p1 = lds(row + o1[e]);
-            L[e] = fmaf(ct[e], lds4(row + o1[e]) - p1, p1 - zref);
+            L[e] = fmaf(ct[e], lds(row + o2[e]) - p1, p1 - zref);
         }
     };
 
@@ -274,23 +300,36 @@ catmull_rom_gather_kernel(const float* __restrict__ in, float* __restrict__ out,
 
 }  // namespace
 
+extern bool g_bilinear_tma;    // bilinear.cu
+
 int launch_catmull_rom(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
                        cudaStream_t stream)
 {
     const AxisMap ax = axis_x(in, out), ay = axis_y(in, out);
     constexpr int CPT = 4, TH = 32, TW = CPT * kThreads;
     const long long fw = footprint_bound(ax, TW) + 2, fh = footprint_bound(ay, TH) + 2;
-    const long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
+    long long smem = ((fw + 6) & ~3LL) * fh * (long long)sizeof(float);
+    CUtensorMap tmap;
+    memset(&tmap, 0, sizeof(tmap));
+    const long long nbox = (fw + 3 + kBoxW - 1) / kBoxW;
+    const long long smem_tma = nbox * fh * kBoxW * (long long)sizeof(float);
+    bool use_tma = g_bilinear_tma && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (in.nx & 3) == 0 && fh <= 256 &&
+                   smem_tma <= 160 * 1024 && in.nx >= kBoxW;
+    if (use_tma) use_tma = tensor_map_2d(&tmap, d_in, in.nx, in.ny, kBoxW, (int)fh) == BATHY_OK;
+    if (use_tma) smem = smem_tma;
     if (smem <= 160 * 1024 && (out.ny + TH - 1) / TH <= 65535) {
         static DeviceOnce once;
         const int rc = once_per_device(once, []() -> int {
-            BATHY_CUDA_TRY(cudaFuncSetAttribute(catmull_rom_tiled_kernel<CPT, TH>,
+            BATHY_CUDA_TRY(cudaFuncSetAttribute(catmull_rom_tiled_kernel<CPT, TH, true>,
+                                                cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+            BATHY_CUDA_TRY(cudaFuncSetAttribute(catmull_rom_tiled_kernel<CPT, TH, false>,
                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
             return (int)BATHY_OK;
         });
         if (rc) return rc;
         dim3 grid((out.nx + TW - 1) / TW, (out.ny + TH - 1) / TH);
-        catmull_rom_tiled_kernel<CPT, TH><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay);
+        if (use_tma) catmull_rom_tiled_kernel<CPT, TH, true><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay, tmap, (int)fh);
+        else         catmull_rom_tiled_kernel<CPT, TH, false><<<grid, kThreads, (size_t)smem, stream>>>(d_in, d_out, ax, ay, tmap, 0);
     } else {
         dim3 grid((out.nx + kThreads - 1) / kThreads, out.ny < 65535 ? out.ny : 65535);
         catmull_rom_gather_kernel<<<grid, kThreads, 0, stream>>>(d_in, d_out, ax, ay);
