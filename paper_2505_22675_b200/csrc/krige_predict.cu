@@ -71,7 +71,7 @@ struct __align__(16) WarpSmem : SolveSmem<K, G> {
     int32_t  cid[S::CAP];                       //             original index
     uint16_t hist[kBuckets + 1][32];            // per-lane key histogram (column = lane)
     uint16_t nbl[K][S::NBLP];                   // per-lane neighbour list: candidate slots
-    uint16_t crit[kCrit][32];                   // per-lane candidates of the critical bucket
+    uint16_t crit[kCrit][32];                   // per-lane candidates of the critical bucket (the last row is a dump slot)
 };
 
 // Reading K2: key = fmaf(ddx, ddx, ddy*ddy) in fp32, ddx = xq - x_i, ddy = yq - y_i.
@@ -233,17 +233,22 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     for (int c = 0; c < n_c; c += 2) {
         float k0, k1; int b0, b1;
         keys2(c, k0, k1, b0, b1);
-        if (k0 <= hi) {
-            if (b0 < bstar) { ws.nbl[cnt][lane] = (uint16_t)c; ++cnt; }
-            else if (b0 == bstar) { if (ncrit < kCrit) ws.crit[ncrit][lane] = (uint16_t)c; ++ncrit; }
-        }
-        if (k1 <= hi) {
-            if (b1 < bstar) { ws.nbl[cnt][lane] = (uint16_t)(c + 1); ++cnt; }
-            else if (b1 == bstar) { if (ncrit < kCrit) ws.crit[ncrit][lane] = (uint16_t)(c + 1); ++ncrit; }
+        // branch-free: the slot is written unconditionally and only kept (the counter advanced) when the candidate
+        // qualifies -- the next candidate overwrites it otherwise.  cnt <= below < k, so nbl[cnt] is inside the list;
+        // the last row of the critical list is its dump slot: the list holds at most kCrit - 1 candidates.
+        {
+            const bool t0 = (k0 <= hi) && (b0 < bstar), c0 = (k0 <= hi) && (b0 == bstar);
+            ws.nbl[cnt][lane] = (uint16_t)c;
+            ws.crit[min(ncrit, kCrit - 1)][lane] = (uint16_t)c;
+            cnt += t0 ? 1 : 0; ncrit += c0 ? 1 : 0;
+            const bool t1 = (k1 <= hi) && (b1 < bstar), c1 = (k1 <= hi) && (b1 == bstar);
+            ws.nbl[cnt][lane] = (uint16_t)(c + 1);
+            ws.crit[min(ncrit, kCrit - 1)][lane] = (uint16_t)(c + 1);
+            cnt += t1 ? 1 : 0; ncrit += c1 ? 1 : 0;
         }
     }
     const int need = k - below;                            // >= 1 candidates of the critical bucket
-    if (ncrit <= kCrit) {
+    if (ncrit < kCrit) {
         for (int e = 0; e < ncrit; ++e) {                  // rank by (key, index) inside the bucket
             const int ce = ws.crit[e][lane];
             const float2 xe = make_float2(ws.cx[ce], ws.cy[ce]);
