@@ -237,11 +237,11 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
         // qualifies -- the next candidate overwrites it otherwise.  cnt <= below < k, so nbl[cnt] is inside the list;
         // the last row of the critical list is its dump slot: the list holds at most kCrit - 1 candidates.
         {
-            const bool t0 = (k0 <= hi) && (b0 < bstar), c0 = (k0 <= hi) && (b0 == bstar);
+            const bool t0 = b0 < bstar, c0 = (b0 == bstar) && (k0 <= hi);       // (b < bstar <= 32 implies key < hi)
             ws.nbl[cnt][lane] = (uint16_t)c;
             ws.crit[min(ncrit, kCrit - 1)][lane] = (uint16_t)c;
             cnt += t0 ? 1 : 0; ncrit += c0 ? 1 : 0;
-            const bool t1 = (k1 <= hi) && (b1 < bstar), c1 = (k1 <= hi) && (b1 == bstar);
+            const bool t1 = b1 < bstar, c1 = (b1 == bstar) && (k1 <= hi);
             ws.nbl[cnt][lane] = (uint16_t)(c + 1);
             ws.crit[min(ncrit, kCrit - 1)][lane] = (uint16_t)(c + 1);
             cnt += t1 ? 1 : 0; ncrit += c1 ? 1 : 0;
