@@ -202,20 +202,37 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     // (The caller pads an odd list with a candidate at infinity: its key is +inf.)
     const u64 xq2 = pack2(xq, xq), yq2 = pack2(yq, yq), neg1 = pack2(-1.0f, -1.0f);
     const u64 sc2 = pack2(scale, scale), mg2 = pack2(12582912.0f, 12582912.0f);
-    auto keys2 = [&](int c, float& k0, float& k1, int& b0, int& b1) {
-        const u64 X = *reinterpret_cast<const u64*>(&ws.cx[c]), Y = *reinterpret_cast<const u64*>(&ws.cy[c]);
+    // keys and buckets of the candidate pair (X, Y) = (cx[c..c+1], cy[c..c+1])
+    auto keys2 = [&](u64 X, u64 Y, float& k0, float& k1, int& b0, int& b1) {
         const u64 dx = ffma2(X, neg1, xq2), dy = ffma2(Y, neg1, yq2);
         const u64 kk = ffma2(dx, dx, fmul2(dy, dy));
         const u64 bb = ffma2(kk, sc2, mg2);
         k0 = lo_of(kk); k1 = hi_of(kk);
         b0 = __float_as_int(lo_of(bb)) - 0x4B400000; b1 = __float_as_int(hi_of(bb)) - 0x4B400000;
     };
+    auto ldpair = [&](int c, u64& X, u64& Y) {
+        X = *reinterpret_cast<const u64*>(&ws.cx[c]); Y = *reinterpret_cast<const u64*>(&ws.cy[c]);
+    };
+    // Both passes are software-pipelined by hand: the next pair's coordinates are loaded BEFORE this pair's
+    // shared-memory stores (the compiler does not move a load above a store it cannot prove disjoint, and the
+    // loop would otherwise pay a full shared-memory round trip per pair), and the two histogram counters of a pair
+    // are read together.  (Reading one pair past the list is harmless: the arrays are followed by others.)
+    {
+        u64 X, Y;
+        ldpair(0, X, Y);
 #pragma unroll 2
-    for (int c = 0; c < n_c; c += 2) {
-        float k0, k1; int b0, b1;
-        keys2(c, k0, k1, b0, b1);
-        if (k0 <= hi) ws.hist[b0][lane] += (uint16_t)1;
-        if (k1 <= hi) ws.hist[b1][lane] += (uint16_t)1;
+        for (int c = 0; c < n_c; c += 2) {
+            u64 Xn, Yn;
+            ldpair(c + 2, Xn, Yn);
+            float k0, k1; int b0, b1;
+            keys2(X, Y, k0, k1, b0, b1);
+            const bool in0 = k0 <= hi, in1 = k1 <= hi;
+            const int s0 = in0 ? b0 : 0, s1 = in1 ? b1 : 0;                // out of range: a harmless read of bucket 0
+            const unsigned h0 = ws.hist[s0][lane], h1 = ws.hist[s1][lane];
+            if (in0) ws.hist[s0][lane] = (uint16_t)(h0 + 1u);
+            if (in1) ws.hist[s1][lane] = (uint16_t)(((in0 && s1 == s0) ? h0 + 1u : h1) + 1u);
+            X = Xn; Y = Yn;
+        }
     }
     // the bucket that holds the k-th key
     int bstar = kBuckets + 1, below = 0, cum = 0;
@@ -229,14 +246,18 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     if (bstar > kBuckets) return false;
     // pass 2: everything below the critical bucket is a neighbour; the critical bucket is listed
     int cnt = 0, ncrit = 0;
+    {
+        u64 X, Y;
+        ldpair(0, X, Y);
 #pragma unroll 2
-    for (int c = 0; c < n_c; c += 2) {
-        float k0, k1; int b0, b1;
-        keys2(c, k0, k1, b0, b1);
-        // branch-free: the slot is written unconditionally and only kept (the counter advanced) when the candidate
-        // qualifies -- the next candidate overwrites it otherwise.  cnt <= below < k, so nbl[cnt] is inside the list;
-        // the last row of the critical list is its dump slot: the list holds at most kCrit - 1 candidates.
-        {
+        for (int c = 0; c < n_c; c += 2) {
+            u64 Xn, Yn;
+            ldpair(c + 2, Xn, Yn);
+            float k0, k1; int b0, b1;
+            keys2(X, Y, k0, k1, b0, b1);
+            // branch-free: the slot is written unconditionally and only kept (the counter advanced) when the candidate
+            // qualifies -- the next candidate overwrites it otherwise.  cnt <= below < k, so nbl[cnt] is inside the list;
+            // the last row of the critical list is its dump slot: the list holds at most kCrit - 1 candidates.
             const bool t0 = b0 < bstar, c0 = (b0 == bstar) && (k0 <= hi);       // (b < bstar <= 32 implies key < hi)
             ws.nbl[cnt][lane] = (uint16_t)c;
             ws.crit[min(ncrit, kCrit - 1)][lane] = (uint16_t)c;
@@ -245,6 +266,7 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
             ws.nbl[cnt][lane] = (uint16_t)(c + 1);
             ws.crit[min(ncrit, kCrit - 1)][lane] = (uint16_t)(c + 1);
             cnt += t1 ? 1 : 0; ncrit += c1 ? 1 : 0;
+            X = Xn; Y = Yn;
         }
     }
     const int need = k - below;                            // >= 1 candidates of the critical bucket
