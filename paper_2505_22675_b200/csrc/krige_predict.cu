@@ -220,7 +220,7 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     {
         u64 X, Y;
         ldpair(0, X, Y);
-#pragma unroll 2
+#pragma unroll 4
         for (int c = 0; c < n_c; c += 2) {
             u64 Xn, Yn;
             ldpair(c + 2, Xn, Yn);
@@ -249,7 +249,7 @@ __device__ __forceinline__ bool select_per_lane(const PredictParams& p, WarpSmem
     {
         u64 X, Y;
         ldpair(0, X, Y);
-#pragma unroll 2
+#pragma unroll 4
         for (int c = 0; c < n_c; c += 2) {
             u64 Xn, Yn;
             ldpair(c + 2, Xn, Yn);
