@@ -124,7 +124,10 @@ BATHY_API int interp_spline(const float* d_in, grid_geom_t in, float* d_out, gri
  * (kriging with duplicates is singular -- such nodes come out NaN, see krige_predict).
  * cell_size: edge of a square cell in the units of x/y; 0 = automatic (about 8 soundings per cell).  A
  * performance knob only: results do not depend on it.  The library enlarges it when the cell grid would
- * exceed 4 cells per sounding or 2^26 cells.
+ * exceed 4 cells per sounding or 2^26 cells.  The build orders the soundings of a cell by original index with a
+ * rank count that is quadratic in the cell's population: fine at the ~8 soundings per cell of the automatic size
+ * on survey-like data, slow when a caller's cell size (or extreme clustering) puts more than ~10^4 soundings into
+ * one cell.
  * The soundings are copied into library-owned device memory: the caller may free d_x/d_y/d_z once
  * the stream reaches this point.  ENQUEUE ONLY: the bounding box never comes back to the host -- the
  * cell grid is sized by a kernel and lives in a device header that krige_predict reads.  Non-finite
