@@ -77,6 +77,10 @@ def test_config5_full_size_tiles_slab_and_samples():
         else:
             tile = b.krige_predict(idx, tg, w.model, w.range_, w.sill, w.nugget, w.k, failed=failed)
         out[i0:i0 + ny, j0:j0 + nx] = tile
+    # the free invariant of per-node independence: the 64 tiles equal ONE 4096^2 call bit for bit
+    mono = b.krige_predict(idx, g, w.model, w.range_, w.sill, w.nugget, w.k, failed=failed)
+    assert torch.equal(mono, out), "tiled output differs from the monolithic output"
+    del mono
     idx.free()
     assert int(failed.item()) == 0
     got = out.cpu().numpy()
