@@ -334,7 +334,7 @@ __device__ __forceinline__ void write_sorted_nbr(const PredictParams& p, WarpSme
 
 // EX: the krige_predict_ex outputs (kriging variance, ill-conditioning counter) are compiled in
 template <int K, int G, int MODEL, bool EX>
-__global__ void __launch_bounds__(Shape<K, G>::WARPS * 32, 1)
+__global__ void __launch_bounds__(Shape<K, G>::WARPS * 32, Shape<K, G>::CTAS)
 krige_predict_kernel(const PredictParams p)
 {
     using S = Shape<K, G>;

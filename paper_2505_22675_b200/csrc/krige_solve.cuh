@@ -40,7 +40,12 @@ struct Shape {
     static constexpr int R = K / G;             // rows of C per lane
     static constexpr int NB = 32 / G;           // nodes solved by a warp at once
     static constexpr int CAP = (K <= 32) ? 256 : 512;          // shared candidate list
-    static constexpr int WARPS = (K <= 32) ? 16 : 8;           // warps per CTA: one CTA per SM (registers)
+    static constexpr int WARPS = 8;                            // warps per CTA
+    // CTAs per SM (registers: 128 per thread at K <= 32, 255 at K = 64).  Two CTAs of 8 warps instead of one of 16:
+    // each CTA walks the long unrolled solve code together (instruction cache), but the two are in different
+    // phases -- one searches (integer / shared-memory work) while the other solves (FMA work).  Measured on
+    // config 4: 4.88 -> 4.68 ms; four CTAs of 4 warps 4.91 ms; at K = 64 two CTAs of 4 warps 7.2 against 5.8 ms.
+    static constexpr int CTAS = (K <= 32) ? 2 : 1;           // warps per CTA: one CTA per SM (registers)
     static constexpr int NQ = CAP / 32;
     static constexpr int XYS = K + 4;           // float stride of a node's coordinate lists (bank skew)
     // float stride of a node's column buffer: = G (mod 32), so that the NB x G lanes of a warp, each

@@ -55,7 +55,7 @@ struct __align__(16) WindowSmem : SolveSmem<K, G> {
 };
 
 template <int K, int G, int MODEL>
-__global__ void __launch_bounds__(Shape<K, G>::WARPS * 32, 1)
+__global__ void __launch_bounds__(Shape<K, G>::WARPS * 32, Shape<K, G>::CTAS)
 krige_window_kernel(const WindowParams p)
 {
     using S = Shape<K, G>;
@@ -175,7 +175,7 @@ int launch_window_one(const WindowParams& p, cudaStream_t stream)
     int dev = 0, sms = kSMs;
     BATHY_CUDA_TRY(cudaGetDevice(&dev));
     BATHY_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    krige_window_kernel<K, G, MODEL><<<sms, Shape<K, G>::WARPS * 32, smem, stream>>>(p);   // persistent: one CTA per SM
+    krige_window_kernel<K, G, MODEL><<<sms * Shape<K, G>::CTAS, Shape<K, G>::WARPS * 32, smem, stream>>>(p);   // persistent: the CTAs one SM holds
     count_launch();
     return launch_status();
 }
