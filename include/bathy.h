@@ -49,7 +49,8 @@ typedef enum {
     BATHY_ERR_WORKSPACE     = -5,   /* workspace NULL or smaller than *_workspace_bytes() */
     BATHY_ERR_CUDA          = -6,   /* a CUDA runtime call failed (no device, out of memory, launch error) */
     BATHY_ERR_SIZE          = -7,   /* n<1 or n>2^31-1 soundings, or a grid with more than 2^31-1 nodes per row/column */
-    BATHY_ERR_INDEX         = -8    /* index handle NULL or not built by krige_build_index */
+    BATHY_ERR_INDEX         = -8,   /* index handle NULL or not built by krige_build_index */
+    BATHY_ERR_SCRATCH       = -9    /* interp_krige_window_noalloc: the grid has more than BATHY_NOALLOC_MAX_CELLS cells */
 } bathy_status;
 
 #define BATHY_MAX_K 64
@@ -221,6 +222,39 @@ typedef struct {
 } krige_window_t;
 BATHY_API int interp_krige_window(const float* d_in, grid_geom_t g, krige_window_t win, variogram_t vg,
                         float* d_out, uint8_t* d_how_or_null, int64_t* d_failed_or_null, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * interp_krige_window_noalloc -- interp_krige_window for callers that must not allocate device memory while they
+ * run.  Same arguments, same operation, same kernels and the same results as interp_krige_window; the only
+ * difference is where the scratch (the list of hole cells and its counter) lives: in a fixed array inside the
+ * library's device image instead of memory drawn from the stream's pool.  The call issues no cudaMalloc, cudaFree,
+ * cudaMallocAsync, cudaFreeAsync or any other allocating routine; d_in, d_out, d_how and d_failed are the
+ * caller's, as everywhere in this header.
+ *
+ * Meant for: the vehicle's real-time mapping loop, which hands out its whole device-memory budget before the dive
+ * and then may not ask the driver for more (an allocation in the middle of a survey line can fail, and cudaMalloc /
+ * cudaFree stall every stream of the device while they run); host programs whose own allocator has reserved the
+ * GPU, so that a driver allocation behind its back competes with it; and devices or driver configurations without
+ * stream-ordered memory pools, where interp_krige_window itself returns BATHY_ERR_CUDA.
+ *
+ * Limit: g.nx * g.ny <= BATHY_NOALLOC_MAX_CELLS (2048 x 2048 cells); a larger grid is refused with
+ * BATHY_ERR_SCRATCH before anything is enqueued -- tile the grid (overlapping the tiles by win.half cells), or use
+ * interp_krige_window.  Cost: the array takes 16 MiB (4 bytes per cell + 256) of device memory on every GPU on
+ * which this process loads the library's device code, until the process exits, used or not.
+ *
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, with the calling thread's
+ * current device) and sets the kernel attributes, once per device; later calls reuse both.  Make that first call
+ * on each device during start-up, outside of any stream capture.
+ *
+ * Sharing: there is ONE array per device and every call on that device uses it.  Calls issued on the same stream
+ * (or ordered by events) are safe -- each call resets the counter on its stream and rewrites the part of the list
+ * it reads; nothing else of the previous call's contents matters.  Two calls whose work can overlap on the GPU
+ * (different streams with no ordering between them, whether from one host thread or several) race on the list and
+ * both results are undefined.  Each process and each device has its own copy.
+ * Enqueue only; errors as interp_krige_window plus BATHY_ERR_SCRATCH. */
+#define BATHY_NOALLOC_MAX_CELLS 4194304
+BATHY_API int interp_krige_window_noalloc(const float* d_in, grid_geom_t g, krige_window_t win, variogram_t vg,
+                                float* d_out, uint8_t* d_how_or_null, int64_t* d_failed_or_null, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Streaming index (the paper's real-time onboard goal).

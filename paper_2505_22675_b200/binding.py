@@ -26,7 +26,8 @@ SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_byt
            "interp_spline_host", "krige_host", "interp_bilinear_host_async", "interp_spline_host_async",
            "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path",
            "krige_predict_ex", "krige_index_create", "krige_index_append", "interp_catmull_rom_host",
-           "interp_catmull_rom_host_async", "bathy_probe_fp32", "interp_krige_window", "bathy_probe_tma"]
+           "interp_catmull_rom_host_async", "bathy_probe_fp32", "interp_krige_window", "bathy_probe_tma",
+           "interp_krige_window_noalloc"]
 
 
 class GridGeom(C.Structure):
@@ -75,6 +76,7 @@ def lib():
         L.krige_index_create.argtypes = [C.c_float] * 5 + [C.c_int64, vp, C.POINTER(vp)]
         L.krige_index_append.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
         L.interp_krige_window.argtypes = [vp, GridGeom, KrigeWindow, Variogram, vp, vp, vp, vp]
+        L.interp_krige_window_noalloc.argtypes = L.interp_krige_window.argtypes
         L.krige_free_index.argtypes = [vp]
         L.krige_free_index.restype = None
         L.krige_free_index_async.argtypes = [vp, vp]
@@ -306,6 +308,35 @@ def interp_krige_window(z: torch.Tensor, geom, model: int, range_: float, sill: 
                                      how.data_ptr() if how is not None else None, _counter(failed, "failed"),
                                      _stream(stream)), "interp_krige_window")
     return (out, how) if want_how else out
+
+
+NOALLOC_MAX_CELLS = 4194304          # BATHY_NOALLOC_MAX_CELLS of include/bathy.h
+
+
+def interp_krige_window_noalloc(z: torch.Tensor, geom, model: int, range_: float, sill: float, nugget: float, half: int = 2,
+                                n_max: int | None = None, n_min: int = 3, *, out: torch.Tensor, how: torch.Tensor | None = None,
+                                failed: torch.Tensor | None = None, stream=None):
+    """interp_krige_window for callers that may not allocate device memory while they run -- a real-time loop
+    whose memory budget was handed out at start-up, or a program whose own allocator owns the GPU.  The library
+    call behind it allocates nothing: its scratch is a fixed 16 MiB array inside libbathy.so's device image, one
+    per GPU, shared by every call (so calls that can overlap on the GPU race -- keep them on one stream).  This
+    wrapper allocates nothing either, which is why `out` (float32 [ny, nx]) is required and `how` (uint8 [ny, nx],
+    optional) is passed in instead of being created here.  Grids above NOALLOC_MAX_CELLS cells raise BathyError
+    (BATHY_ERR_SCRATCH).  Make the first call on each device at start-up, outside of any stream capture: it looks
+    up the array's device address once.  Returns `out`."""
+    g = _geom(geom)
+    _dev_f32(z, "z")
+    _dev_f32(out, "out")
+    assert z.numel() == g.nx * g.ny and out.numel() == g.nx * g.ny and out.data_ptr() != z.data_ptr()
+    if how is not None:
+        assert how.is_cuda and how.dtype == torch.uint8 and how.is_contiguous() and how.numel() == g.nx * g.ny
+    if n_max is None:
+        n_max = (2 * int(half) + 1) ** 2 - 1
+    vg = Variogram(int(model), float(range_), float(sill), float(nugget))
+    _check(lib().interp_krige_window_noalloc(z.data_ptr(), g, KrigeWindow(int(half), int(n_max), int(n_min)), vg,
+                                             out.data_ptr(), how.data_ptr() if how is not None else None,
+                                             _counter(failed, "failed"), _stream(stream)), "interp_krige_window_noalloc")
+    return out
 
 
 def krige_index_create(xmin: float, xmax: float, ymin: float, ymax: float, capacity: int, cell_size: float = 0.0,

@@ -20,6 +20,8 @@ int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, i
 
 int launch_krige_window(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
                         cudaStream_t);
+int launch_krige_window_noalloc(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
+                                cudaStream_t);
 
 extern bool g_bilinear_tma;
 static std::atomic<int64_t> g_launches{0};
@@ -139,6 +141,22 @@ BATHY_API int interp_krige_window(const float* d_in, grid_geom_t g, krige_window
     if (win.half < 1 || win.half > 3 || win.n_max < 1 || win.n_min < 1) return BATHY_ERR_K;
     return launch_krige_window(d_in, g, win.half, win.n_max, win.n_min, vg, d_out, d_how_or_null, d_failed_or_null,
                                static_cast<cudaStream_t>(cuda_stream));
+}
+
+// interp_krige_window with its scratch in a fixed device array of the library (krige_window.cu): for callers that
+// may not allocate device memory while they run (bathy.h says who and why).  Same checks, then the size limit.
+BATHY_API int interp_krige_window_noalloc(const float* d_in, grid_geom_t g, krige_window_t win, variogram_t vg,
+                                float* d_out, uint8_t* d_how_or_null, int64_t* d_failed_or_null, void* cuda_stream)
+{
+    if (!d_in || !d_out) return BATHY_ERR_NULL;
+    int rc = check_in_geom(g);
+    if (rc) return rc;
+    rc = check_variogram(vg);
+    if (rc) return rc;
+    if (win.half < 1 || win.half > 3 || win.n_max < 1 || win.n_min < 1) return BATHY_ERR_K;
+    if ((long long)g.nx * g.ny > (long long)BATHY_NOALLOC_MAX_CELLS) return BATHY_ERR_SCRATCH;
+    return launch_krige_window_noalloc(d_in, g, win.half, win.n_max, win.n_min, vg, d_out, d_how_or_null, d_failed_or_null,
+                                       static_cast<cudaStream_t>(cuda_stream));
 }
 
 BATHY_API int krige_index_create(float xmin, float xmax, float ymin, float ymax, float cell_size, int64_t capacity,
@@ -297,6 +315,7 @@ BATHY_API const char* bathy_strerror(int status)
         case BATHY_ERR_CUDA:      return "CUDA runtime error (no device, out of memory or launch failure)";
         case BATHY_ERR_SIZE:      return "problem size out of range";
         case BATHY_ERR_INDEX:     return "invalid kriging index handle";
+        case BATHY_ERR_SCRATCH:   return "grid larger than the fixed scratch of interp_krige_window_noalloc (BATHY_NOALLOC_MAX_CELLS = 4194304 cells): tile it or call interp_krige_window";
         default:                  return "unknown status";
     }
 }

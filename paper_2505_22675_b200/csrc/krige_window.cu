@@ -223,4 +223,80 @@ int launch_krige_window(const float* d_in, const grid_geom_t& g, int half, int n
     return rc;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// interp_krige_window_noalloc: the same two kernels, with the hole list and its counter in a fixed device array
+// that is part of the library image instead of memory taken from the stream's pool.
+//
+// Who needs this.  On the vehicle the mapping loop runs with a device-memory budget that was handed out in full
+// at start-up: every buffer is allocated before the dive, and a call that asks the driver for more in the middle
+// of a survey line can fail (nothing left), can stall (cudaMalloc / cudaFree wait for the whole device), or can
+// make the pool grow and trim at the caller's synchronisation points -- none of which a ping-rate loop can
+// afford.  The same holds for a host application whose own allocator has reserved the GPU (a driver allocation
+// made behind its back competes with it), and for devices or driver set-ups without stream-ordered memory pools,
+// where interp_krige_window's cudaMallocAsync simply returns an error.  Those callers pass their input and output
+// buffers as always and the library brings the scratch itself.
+//
+// The price: kNoAllocMaxCells * 4 bytes + 256 bytes (16 MiB) of device memory on EVERY GPU whose context loads
+// this library, from the moment the module is loaded until the process exits, whether or not the call is used;
+// and one array per device, shared by all calls -- see the race note at launch_krige_window_noalloc.
+constexpr long long kNoAllocMaxCells = BATHY_NOALLOC_MAX_CELLS;
+static_assert((kNoAllocMaxCells * (long long)sizeof(int32_t)) % 256 == 0, "the counter sits on a 256-byte boundary behind the list");
+// [kNoAllocMaxCells] hole list, then one 256-byte line whose first word is the hole counter.
+static __device__ __align__(256) int32_t g_window_scratch[kNoAllocMaxCells + 64];
+
+// The DEVICE address of g_window_scratch on the current device.  In host code the name `g_window_scratch` is only
+// the host-side handle of the symbol -- handing it to a kernel or to cudaMemsetAsync would pass a host address --
+// so the address is asked for once per device (with that device current) and remembered.  Devices numbered 64 and
+// above are served too, without the cache.
+static int window_scratch_address(int32_t** out)
+{
+    static std::atomic<int32_t*> cached[64];
+    int dev = 0;
+    BATHY_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev >= 0 && dev < 64) {
+        int32_t* p = cached[dev].load(std::memory_order_acquire);
+        if (p) { *out = p; return BATHY_OK; }
+    }
+    int32_t* p = nullptr;
+    BATHY_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_window_scratch));
+    if (!p) return BATHY_ERR_CUDA;
+    if (dev >= 0 && dev < 64) cached[dev].store(p, std::memory_order_release);   // (a racing first call stores the same address)
+    *out = p;
+    return BATHY_OK;
+}
+
+// Calls no cudaMalloc*, cudaFree* or allocating library routine: cudaGetDevice, cudaGetSymbolAddress (first call
+// on a device), one 4-byte cudaMemsetAsync, cudaFuncSetAttribute (first call per window size and device) and two
+// kernel launches.  The hole list keeps whatever the previous call left in it; only the counter has to start at
+// zero, and the scan writes every list entry the solve kernel reads.  All calls on one device use the one array:
+// two calls whose work overlaps on the GPU (different streams without an event between them, or two host threads)
+// corrupt each other's hole list.
+int launch_krige_window_noalloc(const float* d_in, const grid_geom_t& g, int half, int n_max, int n_min, const variogram_t& vg,
+                                float* d_out, uint8_t* d_how, int64_t* d_failed, cudaStream_t stream)
+{
+    const long long n = (long long)g.nx * g.ny;
+    if (n > kNoAllocMaxCells) return BATHY_ERR_SCRATCH;
+    int32_t* d_holes = nullptr;
+    int rc = window_scratch_address(&d_holes);
+    if (rc) return rc;
+    int32_t* d_count = d_holes + kNoAllocMaxCells;
+    BATHY_CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(int32_t), stream));
+    const long long blocks = (n + kScanThreads - 1) / kScanThreads;
+    const int grid = (int)(blocks < (long long)kSMs * 16 ? blocks : (long long)kSMs * 16);
+    window_scan_kernel<<<grid, kScanThreads, 0, stream>>>(d_in, d_out, d_how, n, d_holes, d_count);
+    count_launch();
+    rc = launch_status();
+    if (rc) return rc;
+    WindowParams p;
+    set_variogram(p, vg);
+    p.zhat = d_out; p.var = nullptr; p.failed = reinterpret_cast<unsigned long long*>(d_failed); p.illcond = nullptr;
+    p.in = d_in; p.how = d_how; p.nx = g.nx; p.ny = g.ny; p.dx = g.dx; p.dy = g.dy;
+    const int wn = (2 * half + 1) * (2 * half + 1) - 1;
+    p.half = half; p.n_max = n_max < wn ? n_max : wn; p.n_min = n_min;
+    p.holes = d_holes; p.n_holes = d_count;
+    if (half == 1) return launch_window_shape<8, 8>(p, vg.model, stream);
+    if (half == 2) return launch_window_shape<24, 8>(p, vg.model, stream);
+    return launch_window_shape<48, 16>(p, vg.model, stream);
+}
+
 }  // namespace bathy
