@@ -290,6 +290,38 @@ def krige_methods(B, sw, tiles, reps, stream, fp32, flush=None):
     return res
 
 
+def append_costs(B, sw, reps, stream):
+    """Streaming index (krige_index_create / krige_index_append): ms per append against batch size, into an index
+    that already holds the rest of the survey, with a caller's cell size and room for 8 M soundings -- the case
+    where the cell arrays are sized for the capacity (4 cells per sounding) but the grid in use is small."""
+    import torch
+    n = int(sw.x.shape[0])
+    sx, sy, sz = (torch.from_numpy(a).cuda() for a in (sw.x, sw.y, sw.z))
+    ext = (float(sw.x.min()), float(sw.x.max()), float(sw.y.min()), float(sw.y.max()))
+    res = {"capacity": 8_000_000, "cell_size_m": 6.0, "held_before_append": None, "by_batch": {}}
+    for batch in (1_000, 10_000, 100_000):
+        held = n - batch
+        idx = B.krige_index_create(*ext, capacity=8_000_000, cell_size=6.0)
+        B.krige_index_append(idx, sx[:held], sy[:held], sz[:held])
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(max(3, min(reps, 10))):             # each repetition appends the same batch to a fresh copy of the state
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            B.krige_index_append(idx, sx[held:], sy[held:], sz[held:])
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+            idx.free()
+            idx = B.krige_index_create(*ext, capacity=8_000_000, cell_size=6.0)
+            B.krige_index_append(idx, sx[:held], sy[:held], sz[:held])
+            torch.cuda.synchronize()
+        idx.free()
+        res["by_batch"][str(batch)] = {"ms_median": statistics.median(ms), "ms_best": min(ms), "held": held}
+    res["note"] = "an append re-merges the sorted arrays: cost ~ batch + cells in use + soundings held, independent of the capacity"
+    return res
+
+
 _WORKLOAD_CACHE = {}
 
 
@@ -348,6 +380,7 @@ def per_config_table(B, stream, peaks, fp32, reps):
     torch.cuda.empty_cache()
     # config 4 (one call), config 5 (64 tile calls in arrival order)
     table["config4"] = krige_methods(B, cached_workload("soundings", 4), None, reps, stream, fp32, flush=flush)
+    table["config4"]["krige_index_append"] = append_costs(B, cached_workload("soundings", 4), reps, stream)
     w5 = cached_workload("soundings", 5)
     table["config5"] = krige_methods(B, w5, w5.tiles, reps, stream, fp32)
     del flush_buf

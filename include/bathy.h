@@ -15,7 +15,8 @@
  *     drained; `*_host_async` calls only enqueue.
  *   - Return value: 0 (BATHY_OK) or a negative bathy_status.  Argument errors are detected
  *     synchronously and nothing is launched.  No exceptions, no environment variables.  Global state:
- *     the launch counter, the spline path selector, and per-DEVICE one-time setup (kernel attributes;
+ *     the launch counter, the spline path selector with the TMA-staging switch it drives (both atomic; profiling
+ *     knobs, see bathy_set_spline_path), the fixed scratch array of interp_krige_window_noalloc, and per-DEVICE one-time setup (kernel attributes;
  *     the first index call on a device raises the release threshold of that device's default memory
  *     pool to 2 GiB so that stream-ordered scratch is recycled instead of returned to the driver).
  *     Calls on distinct streams are thread-safe, and one process may use several devices (the current
@@ -49,7 +50,7 @@ typedef enum {
     BATHY_ERR_WORKSPACE     = -5,   /* workspace NULL or smaller than *_workspace_bytes() */
     BATHY_ERR_CUDA          = -6,   /* a CUDA runtime call failed (no device, out of memory, launch error) */
     BATHY_ERR_SIZE          = -7,   /* n<1 or n>2^31-1 soundings, or a grid with more than 2^31-1 nodes per row/column */
-    BATHY_ERR_INDEX         = -8,   /* index handle NULL or not built by krige_build_index */
+    BATHY_ERR_INDEX         = -8,   /* index handle NULL, not built by krige_build_index, or built on another device than the current one */
     BATHY_ERR_SCRATCH       = -9    /* interp_krige_window_noalloc: the grid has more than BATHY_NOALLOC_MAX_CELLS cells */
 } bathy_status;
 
@@ -110,7 +111,11 @@ BATHY_API int interp_catmull_rom(const float* d_in, grid_geom_t in, float* d_out
  * M_{i-1} + 4 M_i + M_{i+1} = 6 (z_{i-1} - 2 z_i + z_{i+1}) / h^2 (batched tridiagonal solves);
  * S = A z_i + B z_{i+1} + ((A^3-A) M_i + (B^3-B) M_{i+1}) h^2/6, A = 1-t, B = t.  2-D = the tensor
  * product (rows in x, then columns in y).  Interval location, extent and NaN rules as bilinear.
- * Precondition: d_in holds no NaN (a NaN poisons its whole row and column; not checked).
+ * Precondition: d_in holds no NaN (not checked).  With a NaN in d_in the result is undefined in the sense that it
+ * depends on the implementation path: the NaN spreads through the tridiagonal solves that contain it -- the solve
+ * windows of the fused tile kernel (about 11 knots either side), or the 256-knot segments (+ 32-knot halo) of the
+ * global-solve path -- along its row and its column, and through everything evaluated from those knots; output
+ * nodes further away are unaffected.
  * d_workspace: device scratch of at least interp_spline_workspace_bytes(in, out) bytes, 256-byte
  * aligned, contents undefined on return; may be reused by later calls on the same stream. */
 BATHY_API size_t interp_spline_workspace_bytes(grid_geom_t in, grid_geom_t out);
@@ -160,9 +165,10 @@ BATHY_API int krige_build_index(const float* d_x, const float* d_y, const float*
 BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram_t vg, int32_t k,
                   float* d_zhat, int32_t* d_nbr_or_null, int64_t* d_failed_or_null, void* cuda_stream);
 
-/* Releases an index after synchronising the stream of its last build / append (NOT the device): the
- * caller guarantees that every krige_predict that uses it was issued on that stream or has completed.
- * NULL is a no-op. */
+/* Releases an index once every kernel that reads it has finished.  BLOCKS the host: it waits for the stream of
+ * the last build / append when every krige_predict[_ex] and append of this index was issued on that stream, and
+ * for the whole device as soon as one of them went to any other stream (the library keeps track; the caller need
+ * not).  Safe to call right after a krige_predict on any stream.  NULL is a no-op. */
 BATHY_API void krige_free_index(krige_index_t* idx);
 
 /* Stream-ordered release, no host synchronisation: the index memory returns to the device's memory
@@ -216,7 +222,13 @@ BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variog
  * win.half in [1, 3] (3x3, 5x5 = the paper's, 7x7); win.n_max >= 1 (values above the window size mean "all");
  * win.n_min >= 1.  d_in [g.ny * g.nx] fp32; d_out the same size, fully overwritten, no overlap with d_in.
  * d_how_or_null [g.ny * g.nx] uint8: 0 = valid cell copied, 1..48 = kriged from that many neighbours, 255 =
- * bilinear fallback.  d_failed_or_null as krige_predict.  Enqueue only (scratch comes from the stream's pool). */
+ * bilinear fallback.  d_how is written when the method is chosen, before the solve: how = 1..48 can accompany a NaN
+ * depth when the system turned out singular (that hole is then counted in d_failed).
+ * d_failed_or_null: one int64 device counter, INCREMENTED by the number of holes whose kriging system was not
+ * positive definite (written NaN), as krige_predict.  It counts singular solves ONLY: a hole that stays NaN through
+ * the bilinear fallback (how = 255 with a NaN or off-grid diagonal neighbour -- always the case on the border rows
+ * and columns) is NOT counted; find those with how == 255 and a NaN depth.
+ * Enqueue only (scratch comes from the stream's pool). */
 typedef struct {
     int32_t half, n_max, n_min;
 } krige_window_t;
@@ -265,7 +277,8 @@ BATHY_API int interp_krige_window_noalloc(const float* d_in, grid_geom_t g, krig
  * appended batches.  create + append(A) + append(B) gives bit for bit the index of create + append(A|B),
  * hence identical neighbours and depths.  Both calls only enqueue work.  Appends and the krige_predict
  * calls that use the index must be ordered by the caller (same stream, or events): an append rewrites the
- * buffers the append before it read from.  After an append only nodes within their k-th-neighbour
+ * buffers the append before it read from.  Cost of one append: O(batch + cells of the grid in use + soundings
+ * already held) -- the sorted arrays are re-merged, not O(capacity).  After an append only nodes within their k-th-neighbour
  * distance of the new soundings change: d_changed_bbox_or_null (4 floats on the device: xmin, xmax,
  * ymin, ymax of the batch) tells the caller which tiles to predict again.
  * Errors: BATHY_ERR_SIZE (capacity exceeded, n < 1), BATHY_ERR_INDEX (index not made by krige_index_create). */
@@ -306,7 +319,9 @@ BATHY_API int krige_host_async(const float* h_x, const float* h_y, const float* 
  *     least one solve window wide), else the global-solve path;
  * 1 = fused tile kernel only (BATHY_ERR_GEOMETRY where it does not apply);
  * 2 = global-solve path only (three batched full-length Thomas solves + gather evaluate);
- * 3 = fused tile kernel with the window staged by cp.async instead of the TMA box load (profiling A/B).
+ * 3 = fused tile kernel with the window staged by cp.async instead of the TMA box load (profiling A/B).  Side
+ *     effect: path 3 ALSO turns the TMA staging of interp_bilinear and interp_catmull_rom off (they stage by cp.async
+ *     instead, same results), and paths 0-2 turn it back on -- one process-wide atomic switch for all grid kernels.
  * Both compute the same natural bicubic spline; DESIGN.md "Spline window bound" gives the bound on
  * their difference (8.2e-7 x depth range per direction). */
 BATHY_API int bathy_set_spline_path(int path);

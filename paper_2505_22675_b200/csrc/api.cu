@@ -23,7 +23,7 @@ int launch_krige_window(const float*, const grid_geom_t&, int, int, int, const v
 int launch_krige_window_noalloc(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
                                 cudaStream_t);
 
-extern bool g_bilinear_tma;
+extern std::atomic<bool> g_bilinear_tma;
 static std::atomic<int64_t> g_launches{0};
 static std::atomic<int> g_spline_path{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
@@ -324,7 +324,7 @@ BATHY_API int bathy_set_spline_path(int path)
 {
     if (path < 0 || path > 3) return BATHY_ERR_GEOMETRY;
     g_spline_path.store(path);
-    g_bilinear_tma = (path != 3);
+    g_bilinear_tma.store(path != 3, std::memory_order_relaxed);
     return BATHY_OK;
 }
 

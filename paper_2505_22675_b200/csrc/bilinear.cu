@@ -217,7 +217,7 @@ bilinear_gather_kernel(const float* __restrict__ in, float* __restrict__ out, Ax
 
 }  // namespace
 
-bool g_bilinear_tma = true;   // A/B switch (bathy_set_spline_path(3) turns the TMA staging of the grid kernels off)
+std::atomic<bool> g_bilinear_tma{true};   // A/B switch (bathy_set_spline_path(3) turns the TMA staging of the grid kernels off)
 
 int launch_bilinear(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
                     cudaStream_t stream)
@@ -232,7 +232,7 @@ int launch_bilinear(const float* d_in, const grid_geom_t& in, float* d_out, cons
     memset(&tmap, 0, sizeof(tmap));
     const long long nbox = (fw + 3 + kBoxW - 1) / kBoxW;
     const long long smem_tma = nbox * fh * kBoxW * (long long)sizeof(float);
-    bool use_tma = g_bilinear_tma && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (in.nx & 3) == 0 && fh <= 256 &&
+    bool use_tma = g_bilinear_tma.load(std::memory_order_relaxed) && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (in.nx & 3) == 0 && fh <= 256 &&
                    smem_tma <= 160 * 1024 && in.nx >= kBoxW;
     if (use_tma) use_tma = tensor_map_2d(&tmap, d_in, in.nx, in.ny, kBoxW, (int)fh) == BATHY_OK;
     if (use_tma) smem = smem_tma;

@@ -300,7 +300,7 @@ catmull_rom_gather_kernel(const float* __restrict__ in, float* __restrict__ out,
 
 }  // namespace
 
-extern bool g_bilinear_tma;    // bilinear.cu
+extern std::atomic<bool> g_bilinear_tma;    // bilinear.cu
 
 int launch_catmull_rom(const float* d_in, const grid_geom_t& in, float* d_out, const grid_geom_t& out,
                        cudaStream_t stream)
@@ -313,7 +313,7 @@ int launch_catmull_rom(const float* d_in, const grid_geom_t& in, float* d_out, c
     memset(&tmap, 0, sizeof(tmap));
     const long long nbox = (fw + 3 + kBoxW - 1) / kBoxW;
     const long long smem_tma = nbox * fh * kBoxW * (long long)sizeof(float);
-    bool use_tma = g_bilinear_tma && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (in.nx & 3) == 0 && fh <= 256 &&
+    bool use_tma = g_bilinear_tma.load(std::memory_order_relaxed) && (reinterpret_cast<uintptr_t>(d_in) & 15) == 0 && (in.nx & 3) == 0 && fh <= 256 &&
                    smem_tma <= 160 * 1024 && in.nx >= kBoxW;
     if (use_tma) use_tma = tensor_map_2d(&tmap, d_in, in.nx, in.ny, kBoxW, (int)fh) == BATHY_OK;
     if (use_tma) smem = smem_tma;

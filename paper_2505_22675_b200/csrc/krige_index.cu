@@ -139,6 +139,23 @@ __global__ void header_update_kernel(IndexHeader* __restrict__ hdr, const float4
     if (hdr->n > 0 && isfinite(w) && isfinite(h)) hdr->step_hint = (float)sqrt((w > 0 ? w : c) * (h > 0 ? h : c) / (double)hdr->n);
 }
 
+// ---- The cell arrays are allocated for the host-known capacity `cap` (+ 1), but the grid the device sized may be
+//      far smaller (a caller's cell size asks for up to 4 cells per sounding of CAPACITY).  Only entries
+//      [0, ncx*ncy] are ever read -- by the kernels below and by krige_predict -- so the per-append sweeps (zeroing,
+//      scan, add-back) stop there: an append costs O(batch + cells in use + soundings held), not O(capacity).
+__device__ __forceinline__ int64_t cells_in_use(const IndexHeader* __restrict__ hdr, int64_t cap)
+{
+    const int64_t m = (int64_t)hdr->ncx * hdr->ncy + 1;      // entry ncx*ncy holds the total
+    return m < cap ? m : cap;
+}
+
+__global__ void __launch_bounds__(kThreads)
+zero_counts_kernel(int32_t* __restrict__ count, int64_t cap, const IndexHeader* __restrict__ hdr)
+{
+    const int64_t n = cells_in_use(hdr, cap);
+    for (int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x; i < n; i += (int64_t)gridDim.x * kThreads) count[i] = 0;
+}
+
 // ---- histogram of the new soundings per cell
 __global__ void __launch_bounds__(kThreads)
 cell_count_kernel(const float* __restrict__ x, const float* __restrict__ y, int64_t n,
@@ -157,9 +174,15 @@ constexpr int kScanItems = 8;
 constexpr int kScanBlock = kThreads * kScanItems;
 
 __global__ void __launch_bounds__(kThreads)
-scan_block_kernel(const int32_t* __restrict__ in, int32_t* __restrict__ out, int64_t n, int32_t* __restrict__ sums)
+scan_block_kernel(const int32_t* __restrict__ in, int32_t* __restrict__ out, int64_t cap, const IndexHeader* __restrict__ hdr,
+                  int32_t* __restrict__ sums)
 {
     __shared__ int32_t s_warp[kThreads / 32];
+    const int64_t n = cells_in_use(hdr, cap);
+    if ((int64_t)blockIdx.x * kScanBlock >= n) {             // beyond the grid in use: nothing to scan, a zero block sum
+        if (threadIdx.x == 0) sums[blockIdx.x] = 0;
+        return;
+    }
     const int64_t base = (int64_t)blockIdx.x * kScanBlock + (int64_t)threadIdx.x * kScanItems;
     int32_t v[kScanItems];
     int32_t tsum = 0;
@@ -213,24 +236,28 @@ scan_sums_kernel(int32_t* __restrict__ sums, int nb)
     }
 }
 
-// prefix[c] += block offset (the exclusive prefix of the NEW soundings per cell, prefix[n] = total), and
+// prefix[c] += block offset (the exclusive prefix of the NEW soundings per cell, prefix[cap] = total),
+// cursor[c] = prefix[c] (where the scatter puts the next sounding of cell c; overwrites the counts), and
 // start_new[c] = start_old[c] + prefix[c] (start_old == NULL: an empty index)
 __global__ void __launch_bounds__(kThreads)
-scan_add_kernel(int32_t* __restrict__ prefix, int64_t n, const int32_t* __restrict__ sums, int32_t total,
-                const int32_t* __restrict__ start_old, int32_t* __restrict__ start_new)
+scan_add_kernel(int32_t* __restrict__ prefix, int64_t cap, const IndexHeader* __restrict__ hdr, const int32_t* __restrict__ sums,
+                int32_t total, const int32_t* __restrict__ start_old, int32_t* __restrict__ start_new, int32_t* __restrict__ cursor)
 {
+    const int64_t n = cells_in_use(hdr, cap);
     const int64_t base = (int64_t)blockIdx.x * kScanBlock;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        prefix[cap] = total;
+        start_new[cap] = total + (start_old ? start_old[cap] : 0);
+    }
+    if (base >= n) return;
     const int32_t off = sums[blockIdx.x];
     for (int e = threadIdx.x; e < kScanBlock; e += kThreads)
         if (base + e < n) {
             const int32_t v = prefix[base + e] + off;
             prefix[base + e] = v;
+            cursor[base + e] = v;
             start_new[base + e] = v + (start_old ? start_old[base + e] : 0);
         }
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        prefix[n] = total;
-        start_new[n] = total + (start_old ? start_old[n] : 0);
-    }
 }
 
 // ---- the soundings already in the index move right by the number of new soundings in the cells before theirs
@@ -386,13 +413,12 @@ int merge_soundings(krige_index* idx, const float* d_x, const float* d_y, const 
     bbox_final_kernel<<<1, 32, 0, stream>>>(d_bb, nb, d_bb + nb);
     if (size_first)
         size_grid_kernel<<<1, 32, 0, stream>>>(d_bb + nb, make_float4(0, 0, 0, 0), 0, (long long)n_new, cell_size, (long long)cells, idx->d_hdr);
-    if (cudaMemsetAsync(d_count, 0, sizeof(int32_t) * (size_t)(cells + 1), stream) != cudaSuccess) { cudaGetLastError(); return BATHY_ERR_CUDA; }
+    zero_counts_kernel<<<grid_for(cells + 1), kThreads, 0, stream>>>(d_count, cells + 1, idx->d_hdr);
     cell_count_kernel<<<nb, kThreads, 0, stream>>>(d_x, d_y, n_new, idx->d_hdr, d_count);
-    scan_block_kernel<<<nsb, kThreads, 0, stream>>>(d_count, d_prefix, cells, d_sums);
+    scan_block_kernel<<<nsb, kThreads, 0, stream>>>(d_count, d_prefix, cells, idx->d_hdr, d_sums);
     scan_sums_kernel<<<1, kThreads, 0, stream>>>(d_sums, nsb);
-    scan_add_kernel<<<nsb, kThreads, 0, stream>>>(d_prefix, cells, d_sums, (int32_t)n_new, start_old, start_dst);
-    if (cudaMemcpyAsync(d_count, d_prefix, sizeof(int32_t) * (size_t)cells, cudaMemcpyDeviceToDevice, stream) != cudaSuccess) { cudaGetLastError(); return BATHY_ERR_CUDA; }
-    int launches = 8 + (size_first ? 1 : 0);
+    scan_add_kernel<<<nsb, kThreads, 0, stream>>>(d_prefix, cells, idx->d_hdr, d_sums, (int32_t)n_new, start_old, start_dst, d_count);
+    int launches = 10 + (size_first ? 1 : 0);   // bbox x2, zero, count, scan x3, scatter, order, header update
     if (n_old > 0) {
         shift_old_kernel<<<grid_for(n_old), kThreads, 0, stream>>>(idx->d_pts, n_old, idx->d_hdr, d_prefix, pts_dst);
         ++launches;
@@ -408,6 +434,7 @@ int merge_soundings(krige_index* idx, const float* d_x, const float* d_y, const 
         int32_t* u = idx->d_cell_start; idx->d_cell_start = idx->d_cell_start_alt; idx->d_cell_start_alt = u;
     }
     idx->n = n_old + n_new;
+    if (stream != idx->stream) __atomic_store_n(&idx->used_elsewhere, 1, __ATOMIC_RELEASE);   // earlier work stays on the old stream
     idx->stream = stream;
     return BATHY_OK;
 }
@@ -458,6 +485,7 @@ int append_index(krige_index* idx, const float* d_x, const float* d_y, const flo
                  float* d_changed, cudaStream_t stream)
 {
     if (!idx->d_pts_alt) return BATHY_ERR_INDEX;           // built by krige_build_index: not appendable
+    if (!index_on_current_device(idx)) return BATHY_ERR_INDEX;
     if (idx->n + n > idx->capacity) return BATHY_ERR_SIZE;
     return merge_soundings(idx, d_x, d_y, d_z, n, false, 0.0f, d_changed, stream);
 }
@@ -466,6 +494,7 @@ int append_index(krige_index* idx, const float* d_x, const float* d_y, const flo
 // synchronises the host, besides krige_free_index).
 int index_header(const krige_index* idx, IndexHeader* out)
 {
+    if (!index_on_current_device(idx)) return BATHY_ERR_INDEX;
     if (cudaMemcpyAsync(out, idx->d_hdr, sizeof(IndexHeader), cudaMemcpyDeviceToHost, idx->stream) != cudaSuccess ||
         cudaStreamSynchronize(idx->stream) != cudaSuccess) { cudaGetLastError(); return BATHY_ERR_CUDA; }
     return BATHY_OK;
@@ -477,7 +506,11 @@ void free_index(krige_index* idx)
     int cur = 0;
     cudaGetDevice(&cur);
     if (cur != idx->device) cudaSetDevice(idx->device);
-    cudaStreamSynchronize(idx->stream);                    // the stream of the last build / append
+    // Every kernel that reads the index must have finished before its memory returns to the pool.  When all of them
+    // were issued on the stream of the last build / append, waiting for that stream is enough; once a krige_predict
+    // (or an earlier append) went to another stream, only the device-wide wait is safe.
+    if (__atomic_load_n(&idx->used_elsewhere, __ATOMIC_ACQUIRE)) cudaDeviceSynchronize();
+    else cudaStreamSynchronize(idx->stream);
     cudaGetLastError();
     release_index_memory(idx, idx->stream);
     if (cur != idx->device) cudaSetDevice(cur);

@@ -30,6 +30,8 @@ struct krige_index {
     int      device;            // CUDA device the memory lives on
     bathy::IndexHeader* d_hdr;  // device header (what the kernels read)
     cudaStream_t stream;        // stream of the last build / append (krige_free_index waits on it)
+    int      used_elsewhere;    // set once work that reads the index was issued on any other stream: krige_free_index
+                                // then waits for the whole device (written with __atomic_store_n: predicts may run concurrently)
     float4*  d_pts;             // [capacity] cell-sorted (x, y, z, original index as int bits)
     float4*  d_pts_alt;         // [capacity] second buffer of an appendable index (ping-pong), else NULL
     int32_t* d_cell_start;      // [cells_cap + 1] exclusive prefix of the per-cell counts
@@ -38,6 +40,14 @@ struct krige_index {
 
 namespace bathy {
 constexpr uint32_t kIndexMagic = 0x4b524947u;   // "KRIG"
+
+// An index belongs to the device it was built on: with another device current, its pointers are foreign and a
+// launch would fault with a sticky context error instead of a status code.
+inline bool index_on_current_device(const krige_index* idx)
+{
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == idx->device;
+}
 
 // The cell of a coordinate, as the index build computes it (fp32, truncation, clamped).
 __device__ __forceinline__ int cell_of(float v, float vmin, float inv_cell, int nc)

@@ -543,6 +543,8 @@ int launch_shape(const PredictParams& p, int model, cudaStream_t stream)
 int launch_predict(const krige_index* idx, const grid_geom_t& out, const variogram_t& vg, int k,
                    float* d_zhat, float* d_var, int32_t* d_nbr, int64_t* d_failed, int64_t* d_illcond, cudaStream_t stream)
 {
+    if (!index_on_current_device(idx)) return BATHY_ERR_INDEX;
+    if (stream != idx->stream) __atomic_store_n(&const_cast<krige_index*>(idx)->used_elsewhere, 1, __ATOMIC_RELEASE);
     PredictParams p;
     p.pts = idx->d_pts;
     p.cell_start = idx->d_cell_start;

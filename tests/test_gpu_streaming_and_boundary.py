@@ -301,6 +301,53 @@ def test_two_threads_first_calls_on_distinct_streams():
         assert torch.equal(a, c)
 
 
+def test_free_right_after_a_predict_on_another_stream():
+    """krige_free_index is safe right after a krige_predict that went to a stream other than the build's: the
+    library notices the foreign stream and waits for the device before the index memory returns to the pool
+    (with only the build stream awaited, the next stream-ordered allocation could be handed the blocks
+    the running kernel still reads).  The memory is recycled at once by a second build plus a fill of the pool."""
+    b = _bathy()
+    w = W.sounding_config(4, width=400.0, n_target=40000, n_out=512)
+    xt, yt, zt = _dev(w.x, w.y, w.z)
+    args = (w.geom_out, w.model, w.range_, w.sill, w.nugget, w.k)
+    idx = b.krige_build_index(xt, yt, zt)
+    want = b.krige_predict(idx, *args).clone()
+    torch.cuda.synchronize()
+    idx.free()
+    other = torch.cuda.Stream()
+    junk = (xt + 3.0e5, yt - 3.0e5, torch.full_like(zt, 123.0))   # other soundings of the same count
+    for _ in range(3):
+        idx = b.krige_build_index(xt, yt, zt)                  # built on the current stream ...
+        other.wait_stream(torch.cuda.current_stream())
+        got = torch.empty_like(want)
+        b.krige_predict(idx, *args, out=got, stream=other)     # ... read on another one (a few ms of work)
+        idx.free()                                             # must not let go of the memory early
+        idx2 = b.krige_build_index(*junk)                      # same sizes: the pool hands the freed blocks straight back
+        torch.cuda.synchronize()
+        idx2.free()
+        assert torch.equal(got, want)
+
+
+@pytest.mark.skipif(torch.cuda.is_available() and torch.cuda.device_count() < 2, reason="needs two visible devices")
+def test_index_of_another_device_is_refused():
+    b = _bathy()
+    w = W.sounding_config(4, width=120.0, n_target=3600, n_out=64)
+    torch.cuda.set_device(0)
+    idx = b.krige_build_index(*_dev(w.x, w.y, w.z))
+    try:
+        torch.cuda.set_device(1)
+        with pytest.raises(b.BathyError) as e:
+            b.krige_predict(idx, w.geom_out, w.model, w.range_, w.sill, w.nugget, w.k,
+                            out=torch.empty((w.geom_out.ny, w.geom_out.nx), dtype=torch.float32, device="cuda:1"))
+        assert e.value.status == -8                            # BATHY_ERR_INDEX, not a sticky illegal-address error
+        with pytest.raises(b.BathyError):
+            idx.info()
+    finally:
+        torch.cuda.set_device(0)
+    assert idx.info()["n"] == w.x.size
+    idx.free()
+
+
 @pytest.mark.skipif(torch.cuda.is_available() and torch.cuda.device_count() < 2, reason="needs two visible devices")
 def test_second_device_after_the_first_in_one_process():
     b = _bathy()
