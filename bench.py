@@ -186,6 +186,40 @@ def alu_roof(ms, k, n_nodes, fp32):
             "flop_per_node": krige_flops(k)}
 
 
+def measure_link(h_in, h_out, dev, reps=3):
+    """Bare pinned-memory copy rates of this process on this box (cudaMemcpyAsync through torch's copy_, CUDA
+    events): host->device of the step's grid input, device->host of one grid result, and both at once on two
+    streams (the link is full duplex).  These make `e2e` self-explaining: a slow box shows up here, not as a
+    mystery in ms_per_step."""
+    import torch
+    d_in = torch.empty(h_in.shape, dtype=h_in.dtype, device=dev)
+    d_out = torch.empty(h_out.shape, dtype=h_out.dtype, device=dev)
+    s1, s2 = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+    nb_in, nb_out = h_in.numel() * h_in.element_size(), h_out.numel() * h_out.element_size()
+
+    def timed(fn):
+        best = float("inf")
+        for _ in range(reps + 1):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            torch.cuda.synchronize()
+            best = min(best, time.perf_counter() - t0)
+        return best
+
+    def h2d():
+        with torch.cuda.stream(s1):
+            d_in.copy_(h_in, non_blocking=True)
+
+    def d2h():
+        with torch.cuda.stream(s2):
+            h_out.copy_(d_out, non_blocking=True)
+    t_h2d, t_d2h, t_both = timed(h2d), timed(d2h), timed(lambda: (h2d(), d2h()))
+    return {"h2d_gbs": nb_in / t_h2d / 1e9, "d2h_gbs": nb_out / t_d2h / 1e9,
+            "duplex_gbs": (nb_in + nb_out) / t_both / 1e9, "h2d_probe_bytes": nb_in, "d2h_probe_bytes": nb_out,
+            "pinned": bool(h_in.is_pinned() and h_out.is_pinned())}
+
+
 def measure_fp32_peak(B, stream, reps=5):
     """FMA-chain microbenchmark of the library (bathy_probe_fp32): TFLOP/s of scalar FFMA and packed FFMA2."""
     import torch
@@ -565,17 +599,30 @@ def run_ours(args):
             return float(hok[0, 0]) + float(hob[0, 0]) + float(hos[0, 0]) + int(hfail[0])      # the host reads the result
 
         e2e_steps = max(2, min(args.steps, 10))
-        e2e_step()
+        link = measure_link(hz, hob, dev)
+        pool_before = (torch.cuda.mem_get_info(dev)[0])
+        for _ in range(3):                               # warm-up: pool growth, first use of the three streams
+            e2e_step()
         barrier()
+        per_step = []
         te0 = time.perf_counter()
         for _ in range(e2e_steps):
+            ts0 = time.perf_counter()
             e2e_step()
+            per_step.append((time.perf_counter() - ts0) * 1e3)
         barrier()
         e2e_ms = (time.perf_counter() - te0) * 1e3 / e2e_steps
         e2e_ms = sharding.reduce_step_times([e2e_ms], dist, dev)[0]
+        h2d_b, d2h_b = 2 * gi.n * 4 + 3 * sw.x.shape[0] * 4, 2 * n_grid * 4 + n_krige * 4 + 8
+        floor_ms = max(h2d_b / link["h2d_gbs"], d2h_b / link["d2h_gbs"]) / 1e6     # full duplex: the slower direction
         e2e = {"value": world * nodes_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
-               "h2d_bytes_per_step": 2 * gi.n * 4 + 3 * sw.x.shape[0] * 4, "d2h_bytes_per_step": 2 * n_grid * 4 + n_krige * 4 + 8,
-               "steps": e2e_steps,
+               "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b,
+               "steps": e2e_steps, "ms_per_step_each": per_step,
+               "link_gbs": link, "ms_copy_floor": floor_ms, "ms_over_copy_floor": e2e_ms / floor_ms,
+               "device_free_bytes_before_after": [int(pool_before), int(torch.cuda.mem_get_info(dev)[0])],
+               "note": "ms_copy_floor = the step's bytes in the slower direction / the bare pinned copy rate measured in this "
+                       "process just before (link_gbs); a step far above its floor on a fast link is the library's fault, "
+                       "a slow link_gbs is the box's",
                "api": "interp_bilinear_host_async + interp_spline_host_async + krige_host_async on three streams, then stream synchronize (pinned host buffers); no call blocks the host"}
         del hz, hob, hos, hx, hy, hzz, hok
 
@@ -643,6 +690,20 @@ def run_ours(args):
         "gpu_launches": int(n1 - n0),
         "clocks": clocks,
     }
+    if table is not None:
+        # every config's kernels against their rooflines at the top level (the driver's record keeps top-level keys):
+        # kriging k = 32 (config 4) AND k = 64 (config 5, 64 streamed tiles), bilinear / spline of configs 2-3
+        by = {}
+        for cfg, methods in table.items():
+            for mname, e in methods.items():
+                if isinstance(e, dict) and "roofline" in e and "ms_median" in e:
+                    r = e["roofline"]
+                    frac = r["frac_of_measured"] if r.get("frac_of_measured") is not None else r["frac"]
+                    by[f"{cfg}.{mname}"] = {"bound": r["bound"], "achieved": r["achieved"], "unit": r["unit"],
+                                            "peak": r.get("peak_measured") or r["peak"], "frac": frac, "ms_median": e["ms_median"],
+                                            **({"k": e["k"]} if "k" in e else {}),
+                                            **({"cold_l2_frac": e["cold_l2"]["roofline"]["frac"]} if "cold_l2" in e else {})}
+        line["roofline_by_config"] = by
     if e2e is not None:
         line["e2e"] = e2e
     if args.cpu_baseline and world == 1:

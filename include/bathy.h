@@ -17,7 +17,7 @@
  *     synchronously and nothing is launched.  No exceptions, no environment variables.  Global state:
  *     the launch counter, the spline path selector with the TMA-staging switch it drives (both atomic; profiling
  *     knobs, see bathy_set_spline_path), the fixed scratch array of interp_krige_window_noalloc, and per-DEVICE one-time setup (kernel attributes;
- *     the first index call on a device raises the release threshold of that device's default memory
+ *     the first index or host-buffer call on a device raises the release threshold of that device's default memory
  *     pool to 2 GiB so that stream-ordered scratch is recycled instead of returned to the driver).
  *     Calls on distinct streams are thread-safe, and one process may use several devices (the current
  *     device of the calling thread is used; an index belongs to the device it was built on).

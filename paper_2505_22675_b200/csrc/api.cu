@@ -23,6 +23,8 @@ int launch_krige_window(const float*, const grid_geom_t&, int, int, int, const v
 int launch_krige_window_noalloc(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
                                 cudaStream_t);
 
+void pool_keep_warm();           // krige_index.cu: raises the release threshold of the device's default memory pool, once per device
+
 extern std::atomic<bool> g_bilinear_tma;
 static std::atomic<int64_t> g_launches{0};
 static std::atomic<int> g_spline_path{0};
@@ -40,7 +42,7 @@ static int check_variogram(const variogram_t& v)
 struct DevBuf {
     void* p = nullptr;
     cudaStream_t s;
-    explicit DevBuf(cudaStream_t st) : s(st) {}
+    explicit DevBuf(cudaStream_t st) : s(st) { pool_keep_warm(); }   // a grid-only caller gets a warm pool too, not a cold one at every synchronisation
     int alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 1, s) == cudaSuccess ? BATHY_OK : BATHY_ERR_CUDA; }
     ~DevBuf() { if (p) cudaFreeAsync(p, s); }
 };

@@ -321,7 +321,7 @@ inline int grid_for(int64_t n)
 // The default memory pool gives freed blocks back to the driver at every synchronisation unless its
 // release threshold is raised; with it raised, cudaMallocAsync of the index and its scratch is a
 // pointer bump after the first call.  Once per device (bathy.h documents the side effect).
-static void pool_keep_warm()
+void pool_keep_warm()
 {
     static std::atomic<uint64_t> done{0};
     int dev = 0;

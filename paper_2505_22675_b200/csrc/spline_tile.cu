@@ -272,16 +272,26 @@ spline_tile_kernel(const float* __restrict__ in, float* __restrict__ out, AxisMa
             }
         }
         asm volatile("griddepcontrol.wait;" ::: "memory");               // the tables of this call are complete
-        const int Jbeg = __ldg(tbx + bxt), Jend = __ldg(tbx + bxt + 1);   // output nodes of the tile
-        const int Ibeg = __ldg(tby + byt), Iend = __ldg(tby + byt + 1);
+        // The first table reads behind the wait go through ld_behind_wait, NOT __ldg: a non-coherent load
+        // (LDG.CONSTANT) promises data that nobody writes while this grid runs, so ptxas is free to schedule it --
+        // and every load whose address depends on it -- above the wait, where the tables kernel may not have
+        // written the entry yet (it did: the first wave of CTAs then ran on whatever the workspace held before).
+        // Every other table read of this kernel takes its address from these six values and so stays behind them.
+        auto ld_behind_wait = [](const int* p) {
+            int v;
+            asm volatile("ld.global.ca.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+            return v;
+        };
+        const int Jbeg = ld_behind_wait(tbx + bxt), Jend = ld_behind_wait(tbx + bxt + 1);   // output nodes of the tile
+        const int Ibeg = ld_behind_wait(tby + byt), Iend = ld_behind_wait(tby + byt + 1);
         const int offx = w0x & 3;
         const float* s_z = s_zbuf;
         // the warp's band: knot intervals [kja, kjb) of the tile = output rows [rb, re) (rfirst[j]: first
         // output row whose interval is >= j)
         constexpr int TI = (TYI + NW - 1) / NW;                           // knot intervals per warp
         const int kja = warp * TI, kjb = min(min(kja + TI, TYI), nky - 1);
-        const int rb = min(max(__ldg(rfirst + min(j0 + kja, ay.n_in)), Ibeg), Iend);
-        const int re = (kjb > kja) ? min(max(__ldg(rfirst + min(j0 + kjb, ay.n_in)), Ibeg), Iend) : rb;
+        const int rb = min(max(ld_behind_wait(rfirst + min(j0 + kja, ay.n_in)), Ibeg), Iend);
+        const int re = (kjb > kja) ? min(max(ld_behind_wait(rfirst + min(j0 + kjb, ay.n_in)), Ibeg), Iend) : rb;
         if (use_tma) {
             __syncthreads();                                             // the barrier is initialised
             mbar_wait(bar, 0);                                           // the window has landed
