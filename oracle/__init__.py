@@ -36,6 +36,12 @@ class Vgm(C.Structure):
     _fields_ = [("model", C.c_int32), ("range", C.c_double), ("sill", C.c_double), ("nugget", C.c_double)]
 
 
+class Aniso(C.Structure):
+    """Geometric anisotropy of the variogram (oracle.c, oracle_aniso_lag): direction of greatest continuity in degrees
+    counter-clockwise from +x, ratio = range across / range along in (0, 1]."""
+    _fields_ = [("angle_deg", C.c_double), ("ratio", C.c_double)]
+
+
 EXPONENTIAL, SPHERICAL, GAUSSIAN = 0, 1, 2
 _lib = None
 
@@ -72,6 +78,13 @@ def lib():
         L.oracle_krige_points_var.argtypes = [fp, fp, fp, C.c_int64, C.c_void_p, fp, fp, C.c_int64, vp,
                                               C.c_int, dp, dp, ip]
         L.oracle_krige_points_var.restype = C.c_int64
+        ap = C.POINTER(Aniso)
+        L.oracle_aniso_lag.argtypes = [ap, C.c_double, C.c_double]
+        L.oracle_aniso_lag.restype = C.c_double
+        L.oracle_ok_weights_aniso.argtypes = [dp, dp, C.c_int, C.c_double, C.c_double, vp, ap, dp, dp]
+        L.oracle_krige_points_aniso.argtypes = [fp, fp, fp, C.c_int64, C.c_void_p, fp, fp, C.c_int64, vp, ap,
+                                                C.c_int, dp, dp, ip, dp]
+        L.oracle_krige_points_aniso.restype = C.c_int64
         L.oracle_krige_window.argtypes = [fp, gp, C.c_int, C.c_int, C.c_int, vp, dp, C.POINTER(C.c_uint8)]
         L.oracle_krige_window.restype = C.c_int64
         _lib = L
@@ -213,22 +226,37 @@ def lu_solve(A, b):
     return b
 
 
-def ok_weights(px, py, xq, yq, v: Vgm):
-    """K4: (lambda[k], mu) of the gamma-form ordinary-kriging system, dense LU."""
+def aniso(angle_deg: float, ratio: float) -> Aniso:
+    return Aniso(float(angle_deg), float(ratio))
+
+
+def aniso_lag(a: Aniso | None, dx: float, dy: float) -> float:
+    return float(lib().oracle_aniso_lag(C.byref(a) if a is not None else None, float(dx), float(dy)))
+
+
+def ok_weights(px, py, xq, yq, v: Vgm, a: Aniso | None = None):
+    """K4: (lambda[k], mu) of the gamma-form ordinary-kriging system, dense LU (a: anisotropic lags, NEXT-4)."""
     px, py = _f64(px), _f64(py)
     k = px.shape[0]
     lam = np.empty(k)
     mu = C.c_double(0.0)
-    rc = lib().oracle_ok_weights(_p(px, C.c_double), _p(py, C.c_double), k, float(xq), float(yq),
-                                 C.byref(v), _p(lam, C.c_double), C.byref(mu))
+    if a is not None:
+        rc = lib().oracle_ok_weights_aniso(_p(px, C.c_double), _p(py, C.c_double), k, float(xq), float(yq),
+                                           C.byref(v), C.byref(a), _p(lam, C.c_double), C.byref(mu))
+    else:
+        rc = lib().oracle_ok_weights(_p(px, C.c_double), _p(py, C.c_double), k, float(xq), float(yq),
+                                     C.byref(v), _p(lam, C.c_double), C.byref(mu))
     if rc:
         raise ValueError("singular kriging system")
     return lam, mu.value
 
 
 def krige_points(x, y, z, xq, yq, v: Vgm, k: int, buckets: Buckets | None = None,
-                 want_nbr: bool = True, want_lambda: bool = False, want_var: bool = False):
-    """K1-K5 at fp32 query points.  Returns dict(zhat float64 [nq], nbr int32 [nq,k], lam, failed[, var])."""
+                 want_nbr: bool = True, want_lambda: bool = False, want_var: bool = False, a: Aniso | None = None):
+    """K1-K5 at fp32 query points.  Returns dict(zhat float64 [nq], nbr int32 [nq,k], lam, failed[, var]).
+    a: geometric anisotropy of the variogram (NEXT-4; neighbours stay the k nearest by plain distance)."""
+    if a is not None:
+        return _krige_points_aniso(x, y, z, xq, yq, v, a, k, buckets, want_nbr, want_lambda)
     if want_var:
         return _krige_points_var(x, y, z, xq, yq, v, k, buckets, want_nbr)
     x, y, z = _f32(x), _f32(y), _f32(z)
@@ -246,6 +274,24 @@ def krige_points(x, y, z, xq, yq, v: Vgm, k: int, buckets: Buckets | None = None
     if failed < 0:
         raise ValueError(f"oracle_krige_points: {failed}")
     return {"zhat": zhat, "nbr": nbr, "lam": lam, "failed": int(failed)}
+
+
+def _krige_points_aniso(x, y, z, xq, yq, v, a, k, buckets, want_nbr, want_lambda):
+    x, y, z = _f32(x), _f32(y), _f32(z)
+    xq, yq = _f32(np.ravel(xq)), _f32(np.ravel(yq))
+    nq = xq.shape[0]
+    zhat, var = np.empty(nq, dtype=np.float64), np.empty(nq, dtype=np.float64)
+    nbr = np.empty((nq, k), dtype=np.int32) if want_nbr else None
+    lam = np.empty((nq, k), dtype=np.float64) if want_lambda else None
+    failed = lib().oracle_krige_points_aniso(
+        _p(x, C.c_float), _p(y, C.c_float), _p(z, C.c_float), x.shape[0],
+        buckets.h if buckets is not None else None,
+        _p(xq, C.c_float), _p(yq, C.c_float), nq, C.byref(v), C.byref(a), int(k),
+        _p(zhat, C.c_double), _p(var, C.c_double), _p(nbr, C.c_int32) if want_nbr else None,
+        _p(lam, C.c_double) if want_lambda else None)
+    if failed < 0:
+        raise ValueError(f"oracle_krige_points_aniso: {failed}")
+    return {"zhat": zhat, "var": var, "nbr": nbr, "lam": lam, "failed": int(failed)}
 
 
 def _krige_points_var(x, y, z, xq, yq, v, k, buckets, want_nbr):

@@ -15,7 +15,10 @@
  * lambda1=0.748755187238, equilateral 1/3, constants, sum(lambda)=1, exactness at data, brute-force
  * kNN vs bucket kNN, LU vs numpy.linalg.solve; Catmull-Rom: C(0)=P1, C(1)=P2, C(1/2)=(-P0+9P1+9P2-P3)/16,
  * quadratics reproduced, NaN/edge fallback = bilinear; kriging variance: two-point closed form 0.148703758152,
- * zero at data, sill (1 + 1/k) for the local mean, C-form LAPACK; Gaussian variogram gamma(a).  No function here is "parity unpinned" against
+ * zero at data, sill (1 + 1/k) for the local mean, C-form LAPACK; Gaussian variogram gamma(a); geometric anisotropy
+ * (tests/test_oracle_aniso.py): lags by hand (3-4-5, the sense of the angle), two-point closed form 0.29421281, equal
+ * weights at d along / ratio x d across, ratio 1 = isotropic, isotropic weights and kriging of points transformed
+ * beforehand, neighbours unchanged.  No function here is "parity unpinned" against
  * mathematics; nothing is pinned against the paper's own tables (they need GEBCO).
  */
 #include <math.h>
@@ -450,6 +453,26 @@ double oracle_variogram(const ora_vgm *v, double h)
     return v->nugget + cp * (1.5 * q - 0.5 * q * q * q);
 }
 
+/* Geometric anisotropy of the variogram ("many variants ... can be easily
+ * implemented on top"; the textbook form, e.g. Cressie, the paper's ref [4]; reading Ani).  The lag vector
+ * (dx, dy) between two locations is expressed in the axes of the anisotropy ellipse -- u along the direction of
+ * greatest continuity, angle_deg counter-clockwise from +x, w across it -- and the across component is stretched by
+ * 1 / ratio, ratio = (range across) / (range along) in (0, 1]:
+ *      u =  cos(t) dx + sin(t) dy,   w = (-sin(t) dx + cos(t) dy) / ratio,   h = sqrt(u^2 + w^2),
+ * so that gamma(h) with the variogram's `range` is the variogram along the major axis and reaches the same value
+ * at `ratio` times the distance across it.  a == NULL: the isotropic lag sqrt(dx^2 + dy^2), exactly as before.
+ * Only the variogram sees this lag: the neighbours are still the k nearest in plain Euclidean distance (K2). */
+typedef struct { double angle_deg, ratio; } ora_aniso;
+
+double oracle_aniso_lag(const ora_aniso *a, double dx, double dy)
+{
+    if (!a) return sqrt(dx * dx + dy * dy);
+    double t = a->angle_deg * (3.14159265358979323846 / 180.0);
+    double u = cos(t) * dx + sin(t) * dy;
+    double w = (-sin(t) * dx + cos(t) * dy) / a->ratio;
+    return sqrt(u * u + w * w);
+}
+
 /* Dense LU with partial pivoting ("Gaussian elimination") of the n x n row-major
  * system A x = b, in place.  Returns -1 when a pivot is smaller in magnitude than tiny. */
 int oracle_lu_solve(double *A, double *b, int n, double tiny)
@@ -484,8 +507,8 @@ int oracle_lu_solve(double *A, double *b, int n, double tiny)
  *      [ Gamma  1 ] [ lambda ]   [ gamma0 ]
  *      [ 1^T    0 ] [   mu   ] = [   1    ],   Gamma_ij = gamma(|p_i - p_j|), gamma0_i = gamma(|q - p_i|)
  * h in float64 from the (fp32-valued) coordinates.  lambda[k], *mu out.  -1 if singular. */
-int oracle_ok_weights(const double *px, const double *py, int k, double xq, double yq,
-                      const ora_vgm *v, double *lambda, double *mu)
+static int ok_weights_impl(const double *px, const double *py, int k, double xq, double yq,
+                           const ora_vgm *v, const ora_aniso *a, double *lambda, double *mu)
 {
     int n = k + 1;
     double *A = (double *)malloc(sizeof(double) * (size_t)n * (size_t)n);
@@ -494,12 +517,12 @@ int oracle_ok_weights(const double *px, const double *py, int k, double xq, doub
     for (int i = 0; i < k; ++i) {
         for (int j = 0; j < k; ++j) {
             double dx = px[i] - px[j], dy = py[i] - py[j];
-            A[(size_t)i * n + j] = oracle_variogram(v, sqrt(dx * dx + dy * dy));
+            A[(size_t)i * n + j] = oracle_variogram(v, oracle_aniso_lag(a, dx, dy));
         }
         A[(size_t)i * n + k] = 1.0;
         A[(size_t)k * n + i] = 1.0;
         double dx = xq - px[i], dy = yq - py[i];
-        b[i] = oracle_variogram(v, sqrt(dx * dx + dy * dy));
+        b[i] = oracle_variogram(v, oracle_aniso_lag(a, dx, dy));
     }
     A[(size_t)k * n + k] = 0.0;
     b[k] = 1.0;
@@ -513,6 +536,20 @@ int oracle_ok_weights(const double *px, const double *py, int k, double xq, doub
     return rc;
 }
 
+int oracle_ok_weights(const double *px, const double *py, int k, double xq, double yq,
+                      const ora_vgm *v, double *lambda, double *mu)
+{
+    return ok_weights_impl(px, py, k, xq, yq, v, NULL, lambda, mu);
+}
+
+/* The same system with the anisotropic lag in Gamma and gamma0 (NEXT-4).  ratio outside (0, 1]: -3. */
+int oracle_ok_weights_aniso(const double *px, const double *py, int k, double xq, double yq,
+                            const ora_vgm *v, const ora_aniso *a, double *lambda, double *mu)
+{
+    if (!a || !(a->ratio > 0.0) || a->ratio > 1.0 || !isfinite(a->angle_deg)) return -3;
+    return ok_weights_impl(px, py, k, xq, yq, v, a, lambda, mu);
+}
+
 /* K1-K5 for a list of query points (fp32 coordinates): neighbours (K2), weights (K3, K4) and
  * z_hat = sum lambda_i z_i (K5).  buckets == NULL -> brute-force search.
  * nbr_out [nq*k] (or NULL) receives original indices in ascending (key, index) order;
@@ -521,10 +558,11 @@ int oracle_ok_weights(const double *px, const double *py, int k, double xq, doub
 static int64_t krige_points_impl(const float *x, const float *y, const float *z, int64_t n,
                             const ora_buckets *buckets,
                             const float *xq, const float *yq, int64_t nq,
-                            const ora_vgm *v, int k,
+                            const ora_vgm *v, const ora_aniso *a, int k,
                             double *zhat, int32_t *nbr_out, double *lambda_out, double *var_out)
 {
     if (!x || !y || !z || !xq || !yq || !zhat || k < 1 || k > n || k > 4096) return -1;
+    if (a && (!(a->ratio > 0.0) || a->ratio > 1.0 || !isfinite(a->angle_deg))) return -1;
     if (!(v->range > 0.0) || !(v->sill > 0.0) || v->nugget < 0.0 || v->nugget > v->sill) return -1;
     if (v->model != 0 && v->model != 1 && v->model != 2) return -1;
     int64_t failed = 0;
@@ -537,7 +575,7 @@ static int64_t krige_points_impl(const float *x, const float *y, const float *z,
         double est = NAN, var = NAN, mu = 0.0;
         if (rc == 0) {
             for (int i = 0; i < k; ++i) { px[i] = (double)x[idx[i]]; py[i] = (double)y[idx[i]]; }
-            rc = oracle_ok_weights(px, py, k, (double)xq[q], (double)yq[q], v, lam, &mu);
+            rc = ok_weights_impl(px, py, k, (double)xq[q], (double)yq[q], v, a, lam, &mu);
         }
         if (rc == 0) {
             est = 0.0;
@@ -547,7 +585,7 @@ static int64_t krige_points_impl(const float *x, const float *y, const float *z,
             var = mu;
             for (int i = 0; i < k; ++i) {
                 double dx = (double)xq[q] - px[i], dy = (double)yq[q] - py[i];
-                var += lam[i] * oracle_variogram(v, sqrt(dx * dx + dy * dy));
+                var += lam[i] * oracle_variogram(v, oracle_aniso_lag(a, dx, dy));
             }
         } else {
             failed += 1;
@@ -567,7 +605,7 @@ int64_t oracle_krige_points(const float *x, const float *y, const float *z, int6
                             const ora_vgm *v, int k,
                             double *zhat, int32_t *nbr_out, double *lambda_out)
 {
-    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, k, zhat, nbr_out, lambda_out, NULL);
+    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, NULL, k, zhat, nbr_out, lambda_out, NULL);
 }
 
 /* The same with the kriging variance sigma^2 in var_out [nq]. */
@@ -577,7 +615,19 @@ int64_t oracle_krige_points_var(const float *x, const float *y, const float *z, 
                                 const ora_vgm *v, int k,
                                 double *zhat, double *var_out, int32_t *nbr_out)
 {
-    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, k, zhat, nbr_out, NULL, var_out);
+    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, NULL, k, zhat, nbr_out, NULL, var_out);
+}
+
+/* The same with a geometrically anisotropic variogram (NEXT-4): neighbours by plain distance (K2), lags of the
+ * variogram by oracle_aniso_lag.  var_out, nbr_out, lambda_out may be NULL. */
+int64_t oracle_krige_points_aniso(const float *x, const float *y, const float *z, int64_t n,
+                                  const ora_buckets *buckets,
+                                  const float *xq, const float *yq, int64_t nq,
+                                  const ora_vgm *v, const ora_aniso *a, int k,
+                                  double *zhat, double *var_out, int32_t *nbr_out, double *lambda_out)
+{
+    if (!a) return -1;
+    return krige_points_impl(x, y, z, n, buckets, xq, yq, nq, v, a, k, zhat, nbr_out, lambda_out, var_out);
 }
 
 /* ================================================================== grid-window kriging (hole filling)
