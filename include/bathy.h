@@ -207,6 +207,23 @@ BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variog
                      float* d_zhat, const krige_outputs_t* outputs_or_null, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * krige_predict_aniso -- krige_predict_ex with a geometrically anisotropic variogram ("many
+ * variants ... can be easily implemented on top"; reading Ani).  The lag between two
+ * locations is measured in the axes of the anisotropy ellipse: with t = angle_deg (counter-clockwise from +x, the
+ * direction of greatest continuity),
+ *      u = cos(t) dx + sin(t) dy,   w = (-sin(t) dx + cos(t) dy) / ratio,   h = sqrt(u^2 + w^2),
+ * and gamma(h) is the variogram `vg`, whose `range` is the range ALONG that direction; across it the same values are
+ * reached at ratio times the distance.  ratio = (range across) / (range along) in (0, 1]; ratio = 1 is krige_predict_ex
+ * whatever the angle.  Only the variogram sees this lag: the neighbours are the k nearest soundings by the plain
+ * (key, index) order of krige_predict.  All outputs as krige_predict_ex.
+ * Errors as krige_predict, plus BATHY_ERR_VARIOGRAM for a ratio outside (0, 1] or a non-finite angle. */
+typedef struct {
+    float angle_deg, ratio;
+} krige_aniso_t;
+BATHY_API int krige_predict_aniso(const krige_index_t* idx, grid_geom_t out, variogram_t vg, krige_aniso_t aniso, int32_t k,
+                        float* d_zhat, const krige_outputs_t* outputs_or_null, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * interp_krige_window -- hole filling on a regular grid by ordinary kriging over a window of grid cells, the form
  * of kriging the paper measured: "the implementation in this study uses a 5x5 grid"
  * (PAPER.md:L163); cells removed at random are interpolated back (Grid B, L225-L234).

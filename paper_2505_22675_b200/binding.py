@@ -27,7 +27,7 @@ SYMBOLS = ["interp_bilinear", "interp_catmull_rom", "interp_spline_workspace_byt
            "krige_host_async", "bathy_strerror", "bathy_launch_count", "bathy_set_spline_path",
            "krige_predict_ex", "krige_index_create", "krige_index_append", "interp_catmull_rom_host",
            "interp_catmull_rom_host_async", "bathy_probe_fp32", "interp_krige_window", "bathy_probe_tma",
-           "interp_krige_window_noalloc"]
+           "interp_krige_window_noalloc", "krige_predict_aniso"]
 
 
 class GridGeom(C.Structure):
@@ -41,6 +41,10 @@ class Variogram(C.Structure):
 
 class KrigeOutputs(C.Structure):
     _fields_ = [("d_var", C.c_void_p), ("d_nbr", C.c_void_p), ("d_failed", C.c_void_p), ("d_illcond", C.c_void_p)]
+
+
+class KrigeAniso(C.Structure):
+    _fields_ = [("angle_deg", C.c_float), ("ratio", C.c_float)]
 
 
 class KrigeWindow(C.Structure):
@@ -73,6 +77,7 @@ def lib():
         L.krige_build_index.argtypes = [vp, vp, vp, C.c_int64, C.c_float, vp, C.POINTER(vp)]
         L.krige_predict.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, vp, vp, vp]
         L.krige_predict_ex.argtypes = [vp, GridGeom, Variogram, C.c_int32, vp, C.POINTER(KrigeOutputs), vp]
+        L.krige_predict_aniso.argtypes = [vp, GridGeom, Variogram, KrigeAniso, C.c_int32, vp, C.POINTER(KrigeOutputs), vp]
         L.krige_index_create.argtypes = [C.c_float] * 5 + [C.c_int64, vp, C.POINTER(vp)]
         L.krige_index_append.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp]
         L.interp_krige_window.argtypes = [vp, GridGeom, KrigeWindow, Variogram, vp, vp, vp, vp]
@@ -253,9 +258,10 @@ def _counter(t, name):
 def krige_predict(index: KrigeIndex, gout, model: int, range_: float, sill: float, nugget: float, k: int,
                   out: torch.Tensor | None = None, want_nbr: bool = False, failed: torch.Tensor | None = None,
                   stream=None, want_var: bool = False, var: torch.Tensor | None = None,
-                  illcond: torch.Tensor | None = None):
+                  illcond: torch.Tensor | None = None, aniso: tuple | None = None):
     """PAPER.md:L146-L171.  Returns zhat [ny, nx]; with want_nbr also nbr [ny, nx, k] int32; with want_var (or
-    `var`) also the kriging variance [ny, nx] (krige_predict_ex): (zhat[, nbr][, var])."""
+    `var`) also the kriging variance [ny, nx] (krige_predict_ex): (zhat[, nbr][, var]).  aniso = (angle_deg, ratio):
+    geometrically anisotropic variogram (krige_predict_aniso)."""
     go = _geom(gout)
     dev = torch.device("cuda", torch.cuda.current_device())
     if out is None:
@@ -276,7 +282,11 @@ def krige_predict(index: KrigeIndex, gout, model: int, range_: float, sill: floa
                 t.record_stream(stream)
     vg = Variogram(int(model), float(range_), float(sill), float(nugget))
     fp, ip = _counter(failed, "failed"), _counter(illcond, "illcond")
-    if var is None and ip is None:
+    if aniso is not None:
+        outs = KrigeOutputs(var.data_ptr() if var is not None else None, nbr.data_ptr() if nbr is not None else None, fp, ip)
+        _check(lib().krige_predict_aniso(index.handle, go, vg, KrigeAniso(float(aniso[0]), float(aniso[1])), int(k),
+                                         out.data_ptr(), C.byref(outs), _stream(stream)), "krige_predict_aniso")
+    elif var is None and ip is None:
         _check(lib().krige_predict(index.handle, go, vg, int(k), out.data_ptr(),
                                    nbr.data_ptr() if nbr is not None else None, fp, _stream(stream)), "krige_predict")
     else:

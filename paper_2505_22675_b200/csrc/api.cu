@@ -16,7 +16,7 @@ int index_header(const krige_index*, IndexHeader*);
 void free_index(krige_index*);
 void free_index_async(krige_index*, cudaStream_t);
 int launch_predict(const krige_index*, const grid_geom_t&, const variogram_t&, int, float*, float*, int32_t*, int64_t*,
-                   int64_t*, cudaStream_t);
+                   int64_t*, cudaStream_t, const krige_aniso_t* aniso_or_null);
 
 int launch_krige_window(const float*, const grid_geom_t&, int, int, int, const variogram_t&, float*, uint8_t*, int64_t*,
                         cudaStream_t);
@@ -113,7 +113,7 @@ BATHY_API int krige_predict(const krige_index_t* idx, grid_geom_t out, variogram
     if (rc) return rc;
     if (k < 1 || k > BATHY_MAX_K || (int64_t)k > idx->n) return BATHY_ERR_K;
     return launch_predict(idx, out, vg, k, d_zhat, nullptr, d_nbr_or_null, d_failed_or_null, nullptr,
-                          static_cast<cudaStream_t>(cuda_stream));
+                          static_cast<cudaStream_t>(cuda_stream), nullptr);
 }
 
 BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variogram_t vg, int32_t k,
@@ -129,7 +129,24 @@ BATHY_API int krige_predict_ex(const krige_index_t* idx, grid_geom_t out, variog
     krige_outputs_t o = {nullptr, nullptr, nullptr, nullptr};
     if (outputs_or_null) o = *outputs_or_null;
     return launch_predict(idx, out, vg, k, d_zhat, o.d_var, o.d_nbr, o.d_failed, o.d_illcond,
-                          static_cast<cudaStream_t>(cuda_stream));
+                          static_cast<cudaStream_t>(cuda_stream), nullptr);
+}
+
+BATHY_API int krige_predict_aniso(const krige_index_t* idx, grid_geom_t out, variogram_t vg, krige_aniso_t aniso, int32_t k,
+                        float* d_zhat, const krige_outputs_t* outputs_or_null, void* cuda_stream)
+{
+    if (!idx || idx->magic != kIndexMagic) return BATHY_ERR_INDEX;
+    if (!d_zhat) return BATHY_ERR_NULL;
+    int rc = check_out_geom(out);
+    if (rc) return rc;
+    rc = check_variogram(vg);
+    if (rc) return rc;
+    if (!isfinite(aniso.angle_deg) || !(aniso.ratio > 0.0f) || aniso.ratio > 1.0f) return BATHY_ERR_VARIOGRAM;
+    if (k < 1 || k > BATHY_MAX_K || (int64_t)k > idx->n) return BATHY_ERR_K;
+    krige_outputs_t o = {nullptr, nullptr, nullptr, nullptr};
+    if (outputs_or_null) o = *outputs_or_null;
+    return launch_predict(idx, out, vg, k, d_zhat, o.d_var, o.d_nbr, o.d_failed, o.d_illcond,
+                          static_cast<cudaStream_t>(cuda_stream), &aniso);
 }
 
 BATHY_API int interp_krige_window(const float* d_in, grid_geom_t g, krige_window_t win, variogram_t vg,
@@ -268,7 +285,7 @@ int krige_host_impl(const float* h_x, const float* h_y, const float* h_z, int64_
     rc = build_index(static_cast<const float*>(dx.p), static_cast<const float*>(dy.p), static_cast<const float*>(dz.p),
                      n, cell_size, s, &idx);
     if (rc) return rc;
-    rc = launch_predict(idx, out, vg, k, static_cast<float*>(dout.p), nullptr, nullptr, static_cast<int64_t*>(dfail.p), nullptr, s);
+    rc = launch_predict(idx, out, vg, k, static_cast<float*>(dout.p), nullptr, nullptr, static_cast<int64_t*>(dfail.p), nullptr, s, nullptr);
     if (rc == BATHY_OK) {
         cudaError_t e = cudaMemcpyAsync(h_zhat, dout.p, nout, cudaMemcpyDeviceToHost, s);
         if (e == cudaSuccess && h_failed_or_null)
